@@ -1,0 +1,185 @@
+/*
+ * fasttg.h -- C ABI of libfasttg: temporal-attention message passing over one mini-batch's
+ * sampled temporal subgraph, hand-written for NVIDIA B200 (sm_100a).
+ *
+ * What the library computes (reference = PAPER.md, FAST, arxiv/paper_2607_05095):
+ *   - the compression engine's index triple uni_ID / inv_Idx / CSR ind_ptr (§4.2,
+ *     PAPER.md:287 §5) plus a transposed CSR for the backward gather          -> tg_block_build
+ *   - AGG, h_v = sum_{u in N_in(v)} v_u (§4.3 "Balanced Aggregate", Eq.(1)),
+ *     optionally alpha-weighted                                              -> tg_aggregate_fwd/bwd
+ *   - ESM, the numerically stable edge softmax: max reduction, sum reduction, element-wise division
+ *     per destination (§4.3 "Edge Softmax")                      -> tg_edge_softmax_fwd/bwd
+ *   - per-edge attention logits (DGL gSDDMM, only named at PAPER.md:94)       -> tg_sddmm
+ *   - the three fused into one pass, "forward and backward" -> tg_attn_fused_fwd/bwd
+ *
+ * Conventions shared by every call
+ *   Memory.    Every pointer is a DEVICE pointer unless its comment says HOST.  The library never
+ *              allocates or frees device memory: inputs, outputs, workspaces and the block's index
+ *              arrays belong to the caller and must stay alive until the work enqueued on `stream`
+ *              has finished (block arrays and the block workspace: until tg_block_destroy).
+ *   Layout.    Row-major, contiguous.  Row tensors are [rows, H, D] in the storage dtype (TG_F32 or
+ *              TG_BF16); edge-level tensors are [E, H] float32; all accumulation is float32.
+ *              Base pointers of row tensors must be 16-byte aligned (else TG_ERR_ALIGNMENT).
+ *   Notation.  R destinations (roots), E sampled edges in destination-grouped CSR order, U unique
+ *              source rows, v(e) destination of CSR edge e, r(e) = kv_row[e], N(v) = CSR edges of v.
+ *   Streams.   `stream` is a cudaStream_t passed as void*.  Calls enqueue and return; only
+ *              tg_block_build synchronises the stream (it returns U to the host).
+ *   Errors.    Every call returns a tg_status_t; nothing throws or aborts across the ABI.  Arguments
+ *              are validated before any launch.  tg_last_error() gives thread-local detail text.
+ *   Edge cases. R == 0 or E == 0 is TG_OK.  A zero-degree destination gives O = 0, LSE = -inf,
+ *              dQ = 0 (reading R5).  Inputs must be finite.  Multi-edges are distinct edges.
+ *   Supported (H, D): H in {1,2,4,8,16} with D in {8,16,32,50,64,128} such that H*lanes fit one warp;
+ *              tg_supported() answers for a given (H, D, dtype).  Contains (2,50) (4,32) (8,16) (2,64).
+ *   There is no CPU fallback: without a CUDA device every compute call returns TG_ERR_CUDA.
+ */
+#ifndef FASTTG_H_
+#define FASTTG_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(_WIN32)
+#define TG_API
+#else
+#define TG_API __attribute__((visibility("default")))
+#endif
+
+typedef enum {
+    TG_OK = 0,
+    TG_ERR_INVALID_ARG = 1,  /* null pointer, negative size, out-of-range scalar */
+    TG_ERR_UNSUPPORTED = 2,  /* (H, D, dtype) outside the supported set */
+    TG_ERR_ALIGNMENT = 3,    /* a row tensor's base pointer is not 16-byte aligned */
+    TG_ERR_WORKSPACE = 4,    /* workspace pointer null or too small */
+    TG_ERR_CUDA = 5,         /* a CUDA runtime call failed; text in tg_last_error() */
+    TG_ERR_INTERNAL = 6
+} tg_status_t;
+
+typedef enum { TG_F32 = 0, TG_BF16 = 1 } tg_dtype_t;
+
+typedef void* tg_stream_t; /* cudaStream_t */
+
+/* Host-side handle.  Holds sizes, pointers into caller memory and the internal schedules (which
+ * live in the block workspace).  Created by tg_block_build / tg_block_from_csr. */
+typedef struct tg_block tg_block_t;
+
+TG_API const char* tg_status_string(tg_status_t s);
+TG_API const char* tg_last_error(void);
+TG_API int tg_version(void);
+/* 1 if (H, D, dtype) has a compiled kernel path, else 0. */
+TG_API int tg_supported(int H, int D, tg_dtype_t dtype);
+
+/* ------------------------------------------------------------------------------------------------
+ * Block build: the compression engine's triple + transposed CSR (R7-R10)
+ *
+ * Input: the sampler's COO lists, in any order (E entries):
+ *   root_idx[e]  int32, destination slot in [0,R)       nbr_node[e]  int64, neighbour (source) node id
+ *   edge_id[e]   int64, nullable                        ts[e]        float32, nullable
+ * Output (all caller-allocated, device):
+ *   indptr[R+1]  int32  exclusive prefix sum of bincount(root_idx)            (CSR ind_ptr)
+ *   perm[E]      int32  stable argsort of root_idx: CSR position -> input position
+ *   kv_row[E]    int32  rank of nbr_node[perm[e]] in uniq_node                 (inv_Idx)
+ *   uniq_node[>=E] int64 ascending distinct neighbour ids, U valid entries     (uni_ID)
+ *   t_indptr[>=E+1] int32, t_edge[E] int32, t_dst[E] int32: transposed CSR; row u lists the CSR
+ *                positions e with kv_row[e] == u in ascending order, t_dst[j] = v(t_edge[j])
+ *   eid_csr[E] int64 = edge_id[perm], ts_csr[E] float32 = ts[perm]   (nullable, need their inputs)
+ *   U_host       HOST int64*, written before return
+ * dedup_mode 0: identity rows (U = E, kv_row[e] = e, uniq_node[e] = nbr_node[perm[e]]; K/V are per-edge
+ *               rows [E,H,D]);  dedup_mode 1: dedup by neighbour node id.
+ * All index results are exact integers with exactly one correct value (bit-exact against the oracle).
+ * Errors: TG_ERR_INVALID_ARG (null, R < 0, E < 0, E >= 2^31, R >= 2^31, root_idx out of range ->
+ *         detected on device, reported after the sync), TG_ERR_WORKSPACE, TG_ERR_CUDA.
+ * The workspace must stay alive (and untouched) until tg_block_destroy: the schedules live in it.
+ * ---------------------------------------------------------------------------------------------- */
+TG_API tg_status_t tg_block_workspace_bytes(int64_t R, int64_t E, int dedup_mode, size_t* bytes /*HOST*/);
+
+TG_API tg_status_t tg_block_build(int64_t R, int64_t E,
+                                  const int32_t* root_idx, const int64_t* nbr_node,
+                                  const int64_t* edge_id, const float* ts, int dedup_mode,
+                                  int32_t* indptr, int32_t* perm, int32_t* kv_row, int64_t* uniq_node,
+                                  int32_t* t_indptr, int32_t* t_edge, int32_t* t_dst,
+                                  int64_t* eid_csr, float* ts_csr,
+                                  int64_t* U_host /*HOST*/,
+                                  void* workspace, size_t workspace_bytes, tg_stream_t stream,
+                                  tg_block_t** out /*HOST*/);
+
+/* Wrap index arrays that already exist on the device (e.g. a previous build, or a caller's own
+ * CSR) and build only the internal schedules.  Same ownership rules.  Synchronises the stream.
+ * tg_sched_workspace_bytes gives the workspace size. */
+TG_API tg_status_t tg_sched_workspace_bytes(int64_t R, int64_t E, int64_t U, size_t* bytes /*HOST*/);
+TG_API tg_status_t tg_block_from_csr(int64_t R, int64_t E, int64_t U,
+                                     const int32_t* indptr, const int32_t* kv_row,
+                                     const int32_t* t_indptr, const int32_t* t_edge, const int32_t* t_dst,
+                                     void* workspace, size_t workspace_bytes, tg_stream_t stream,
+                                     tg_block_t** out /*HOST*/);
+
+TG_API tg_status_t tg_block_destroy(tg_block_t* b);
+
+/* Sizes and schedule statistics of a block (HOST outputs; any may be null).
+ * stats[0..7] = dst side {n_small, n_warp, n_cta_items, n_partial_slots}, src side the same. */
+TG_API tg_status_t tg_block_info(const tg_block_t* b, int64_t* R, int64_t* E, int64_t* U, int64_t stats[8]);
+
+/* ------------------------------------------------------------------------------------------------
+ * Unfused operators
+ * ---------------------------------------------------------------------------------------------- */
+
+/* SDDMM (gSDDMM named at PAPER.md:94; R1): s[e,h] = scale * <A[v(e),h,:], B[r(e),h,:]>.
+ * A [R,H,D], B [U,H,D] in `dtype`; s [E,H] float32. */
+TG_API tg_status_t tg_sddmm(const tg_block_t* b, int H, int D, tg_dtype_t dtype,
+                            const void* A, const void* B, float scale, float* s, tg_stream_t stream);
+
+/* ESM forward: alpha[e,h] = exp(s[e,h] - m[v,h]) / l[v,h], m = max over N(v),
+ * l = sum over N(v) of exp(s - m).  s, alpha [E,H] float32; alpha may alias s. */
+TG_API tg_status_t tg_edge_softmax_fwd(const tg_block_t* b, int H, const float* s, float* alpha,
+                                       tg_stream_t stream);
+
+/* ESM backward: ds[e,h] = alpha[e,h] * (dalpha[e,h] - sum_{e' in N(v)} alpha[e',h]*dalpha[e',h]). */
+TG_API tg_status_t tg_edge_softmax_bwd(const tg_block_t* b, int H, const float* alpha, const float* dalpha,
+                                       float* ds, tg_stream_t stream);
+
+/* AGG forward: Y[v,h,:] = sum_{e in N(v)} w[e,h] * X[r(e),h,:]; w == NULL is the paper's
+ * plain neighbour sum.  X [U,H,D], Y [R,H,D] in `dtype`; w [E,H] float32.
+ * ws: tg_attn_workspace_bytes(...).fwd_bytes is sufficient. */
+TG_API tg_status_t tg_aggregate_fwd(const tg_block_t* b, int H, int D, tg_dtype_t dtype,
+                                    const float* w, const void* X, void* Y,
+                                    void* ws, size_t ws_bytes, tg_stream_t stream);
+
+/* AGG backward (the paper scatters with atomics, PAPER.md:219-223 -- here a gather
+ * through the transposed CSR, no float atomics):
+ *   dX[u,h,:] = sum_{e: r(e)=u} w[e,h] * dY[v(e),h,:]          (w == NULL: plain sum)
+ *   dw[e,h]   = <dY[v(e),h,:], X[r(e),h,:]>                    (only if dw != NULL; needs X)
+ * ws: tg_attn_workspace_bytes(...).bwd_bytes is sufficient. */
+TG_API tg_status_t tg_aggregate_bwd(const tg_block_t* b, int H, int D, tg_dtype_t dtype,
+                                    const float* w, const void* X, const void* dY,
+                                    void* dX, float* dw, void* ws, size_t ws_bytes, tg_stream_t stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * Fused attention (SDDMM -> ESM -> alpha-weighted AGG without materialising s or alpha)
+ * ---------------------------------------------------------------------------------------------- */
+TG_API tg_status_t tg_attn_workspace_bytes(const tg_block_t* b, int H, int D, tg_dtype_t dtype,
+                                           size_t* fwd_bytes /*HOST*/, size_t* bwd_bytes /*HOST*/);
+
+/* Forward:  s = scale*<Q[v(e)],K[r(e)]>, alpha = softmax over N(v), O[v] = sum alpha*V[r(e)],
+ *           LSE[v,h] = m + ln l (natural log).  Q,O [R,H,D]; K,V [U,H,D]; LSE [R,H] float32. */
+TG_API tg_status_t tg_attn_fused_fwd(const tg_block_t* b, int H, int D, tg_dtype_t dtype,
+                                     const void* Q, const void* K, const void* V, float scale,
+                                     void* O, float* lse, void* ws, size_t ws_bytes, tg_stream_t stream);
+
+/* Backward for upstream gradient dO:
+ *   delta[v,h] = <dO[v,h,:], O[v,h,:]>;  alpha = exp(s - LSE);  dalpha = <dO[v(e)], V[r(e)]>;
+ *   ds = alpha*(dalpha - delta);  dQ[v] = scale * sum_{N(v)} ds*K[r(e)];
+ *   dK[u] = scale * sum_{r(e)=u} ds*Q[v(e)];  dV[u] = sum_{r(e)=u} alpha*dO[v(e)].
+ * O and lse are the forward's outputs.  dQ [R,H,D]; dK,dV [U,H,D]. */
+TG_API tg_status_t tg_attn_fused_bwd(const tg_block_t* b, int H, int D, tg_dtype_t dtype,
+                                     const void* Q, const void* K, const void* V, const void* O,
+                                     const float* lse, const void* dO, float scale,
+                                     void* dQ, void* dK, void* dV,
+                                     void* ws, size_t ws_bytes, tg_stream_t stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FASTTG_H_ */

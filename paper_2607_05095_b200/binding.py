@@ -1,0 +1,247 @@
+"""Thin ctypes binding over ``libfasttg.so`` (include/fasttg.h).  Argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels; this module turns torch tensors into
+device pointers, allocates outputs / workspaces through torch (the library never allocates), and
+raises ``FastTGError`` on a non-zero status.  There is no CPU fallback: if the shared library is
+missing or no CUDA device is present, calls fail loudly.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libfasttg.so")
+_lib = None
+
+TG_F32, TG_BF16 = 0, 1
+_DTYPES = {torch.float32: TG_F32, torch.bfloat16: TG_BF16}
+
+EXPORTS = [
+    "tg_status_string", "tg_last_error", "tg_version", "tg_supported",
+    "tg_block_workspace_bytes", "tg_block_build", "tg_sched_workspace_bytes", "tg_block_from_csr",
+    "tg_block_destroy", "tg_block_info",
+    "tg_sddmm", "tg_edge_softmax_fwd", "tg_edge_softmax_bwd", "tg_aggregate_fwd", "tg_aggregate_bwd",
+    "tg_attn_workspace_bytes", "tg_attn_fused_fwd", "tg_attn_fused_bwd",
+]
+
+
+class FastTGError(RuntimeError):
+    def __init__(self, status: int, where: str, detail: str):
+        super().__init__(f"{where}: status {status} ({detail})")
+        self.status = status
+
+
+def lib() -> C.CDLL:
+    """Loads libfasttg.so (built by ``paper_2607_05095_b200.build``); raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise FileNotFoundError(f"{_LIB_PATH} not found: run `python -m paper_2607_05095_b200.build` (no CPU fallback exists)")
+        L = C.CDLL(_LIB_PATH)
+        L.tg_status_string.restype = C.c_char_p
+        L.tg_last_error.restype = C.c_char_p
+        for name in EXPORTS:
+            getattr(L, name)  # fail loudly on a missing symbol
+        _lib = L
+    return _lib
+
+
+def _check(st: int, where: str):
+    if st != 0:
+        L = lib()
+        raise FastTGError(st, where, f"{L.tg_status_string(st).decode()}: {L.tg_last_error().decode()}")
+
+
+def _ptr(t):
+    return C.c_void_p(0 if t is None else t.data_ptr())
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _dt(t: torch.Tensor) -> int:
+    try:
+        return _DTYPES[t.dtype]
+    except KeyError:
+        raise TypeError(f"unsupported storage dtype {t.dtype}") from None
+
+
+def _rows(t: torch.Tensor, name: str) -> torch.Tensor:
+    if t.dim() != 3 or not t.is_contiguous() or not t.is_cuda:
+        raise ValueError(f"{name} must be a contiguous CUDA tensor [rows, H, D]")
+    return t
+
+
+def supported(H: int, D: int, dtype: torch.dtype) -> bool:
+    return bool(lib().tg_supported(C.c_int(H), C.c_int(D), C.c_int(_DTYPES[dtype])))
+
+
+class Block:
+    """Destination-grouped CSR block + unique-row remap + transposed CSR (tg_block_build)."""
+
+    def __init__(self):
+        self.handle = C.c_void_p(0)
+        self.R = self.E = self.U = 0
+        self.indptr = self.perm = self.kv_row = self.uniq_node = None
+        self.t_indptr = self.t_edge = self.t_dst = self.eid_csr = self.ts_csr = None
+        self._ws = None
+        self._attn_ws = {}
+
+    def __del__(self):
+        try:
+            if self.handle and _lib is not None:
+                _lib.tg_block_destroy(self.handle)
+                self.handle = C.c_void_p(0)
+        except Exception:
+            pass
+
+    def info(self):
+        R, E, U = C.c_int64(), C.c_int64(), C.c_int64()
+        stats = (C.c_int64 * 8)()
+        _check(lib().tg_block_info(self.handle, C.byref(R), C.byref(E), C.byref(U), stats), "tg_block_info")
+        keys = ["dst_small", "dst_warp", "dst_cta_items", "dst_slots", "src_small", "src_warp", "src_cta_items", "src_slots"]
+        return {"R": R.value, "E": E.value, "U": U.value, **{k: int(v) for k, v in zip(keys, stats)}}
+
+    def attn_workspace(self, H: int, D: int, dtype: torch.dtype):
+        key = (H, D, dtype)
+        if key not in self._attn_ws:
+            fb, bb = C.c_size_t(), C.c_size_t()
+            _check(lib().tg_attn_workspace_bytes(self.handle, C.c_int(H), C.c_int(D), C.c_int(_DTYPES[dtype]),
+                                                 C.byref(fb), C.byref(bb)), "tg_attn_workspace_bytes")
+            dev = self.indptr.device
+            self._attn_ws[key] = (torch.empty(fb.value, dtype=torch.uint8, device=dev),
+                                  torch.empty(bb.value, dtype=torch.uint8, device=dev))
+        return self._attn_ws[key]
+
+
+def block_build(R: int, root_idx: torch.Tensor, nbr_node: torch.Tensor, edge_id: torch.Tensor | None = None,
+                ts: torch.Tensor | None = None, dedup_mode: int = 1) -> Block:
+    """tg_block_build.  root_idx int32 [E], nbr_node int64 [E], edge_id int64 [E] | None, ts float32 [E] | None (CUDA)."""
+    L = lib()
+    dev = root_idx.device
+    if not root_idx.is_cuda:
+        raise ValueError("block_build needs CUDA tensors (no CPU fallback)")
+    E = int(root_idx.shape[0])
+    assert root_idx.dtype == torch.int32 and nbr_node.dtype == torch.int64
+    root_idx, nbr_node = root_idx.contiguous(), nbr_node.contiguous()
+    if edge_id is not None:
+        assert edge_id.dtype == torch.int64
+        edge_id = edge_id.contiguous()
+    if ts is not None:
+        assert ts.dtype == torch.float32
+        ts = ts.contiguous()
+    b = Block()
+    i32 = dict(dtype=torch.int32, device=dev)
+    b.indptr = torch.empty(R + 1, **i32)
+    b.perm = torch.empty(E, **i32)
+    b.kv_row = torch.empty(E, **i32)
+    b.uniq_node = torch.empty(max(E, 1), dtype=torch.int64, device=dev)
+    b.t_indptr = torch.empty(E + 1, **i32)
+    b.t_edge = torch.empty(E, **i32)
+    b.t_dst = torch.empty(E, **i32)
+    b.eid_csr = None if edge_id is None else torch.empty(E, dtype=torch.int64, device=dev)
+    b.ts_csr = None if ts is None else torch.empty(E, dtype=torch.float32, device=dev)
+    nbytes = C.c_size_t()
+    _check(L.tg_block_workspace_bytes(C.c_int64(R), C.c_int64(E), C.c_int(dedup_mode), C.byref(nbytes)), "tg_block_workspace_bytes")
+    b._ws = torch.empty(nbytes.value, dtype=torch.uint8, device=dev)
+    U = C.c_int64()
+    _check(L.tg_block_build(C.c_int64(R), C.c_int64(E), _ptr(root_idx), _ptr(nbr_node), _ptr(edge_id), _ptr(ts),
+                            C.c_int(dedup_mode), _ptr(b.indptr), _ptr(b.perm), _ptr(b.kv_row), _ptr(b.uniq_node),
+                            _ptr(b.t_indptr), _ptr(b.t_edge), _ptr(b.t_dst), _ptr(b.eid_csr), _ptr(b.ts_csr),
+                            C.byref(U), _ptr(b._ws), C.c_size_t(nbytes.value), _stream(), C.byref(b.handle)), "tg_block_build")
+    b.R, b.E, b.U = R, E, int(U.value)
+    b.uniq_node = b.uniq_node[:b.U]
+    b.t_indptr = b.t_indptr[:b.U + 1]
+    return b
+
+
+def block_from_csr(indptr, kv_row, U, t_indptr, t_edge, t_dst) -> Block:
+    """tg_block_from_csr: wrap existing device index arrays, build only the schedules."""
+    L = lib()
+    b = Block()
+    b.indptr, b.kv_row, b.t_indptr, b.t_edge, b.t_dst = (x.contiguous() for x in (indptr, kv_row, t_indptr, t_edge, t_dst))
+    R, E = int(indptr.shape[0]) - 1, int(kv_row.shape[0])
+    nbytes = C.c_size_t()
+    _check(L.tg_sched_workspace_bytes(C.c_int64(R), C.c_int64(E), C.c_int64(U), C.byref(nbytes)), "tg_sched_workspace_bytes")
+    b._ws = torch.empty(nbytes.value, dtype=torch.uint8, device=indptr.device)
+    _check(L.tg_block_from_csr(C.c_int64(R), C.c_int64(E), C.c_int64(U), _ptr(b.indptr), _ptr(b.kv_row), _ptr(b.t_indptr),
+                               _ptr(b.t_edge), _ptr(b.t_dst), _ptr(b._ws), C.c_size_t(nbytes.value), _stream(),
+                               C.byref(b.handle)), "tg_block_from_csr")
+    b.R, b.E, b.U = R, E, int(U)
+    return b
+
+
+def sddmm(b: Block, A: torch.Tensor, B: torch.Tensor, scale: float = 1.0, out: torch.Tensor | None = None) -> torch.Tensor:
+    _rows(A, "A"); _rows(B, "B")
+    H, D = A.shape[1], A.shape[2]
+    s = out if out is not None else torch.empty(b.E, H, dtype=torch.float32, device=A.device)
+    _check(lib().tg_sddmm(b.handle, C.c_int(H), C.c_int(D), C.c_int(_dt(A)), _ptr(A), _ptr(B), C.c_float(scale), _ptr(s), _stream()), "tg_sddmm")
+    return s
+
+
+def edge_softmax_fwd(b: Block, s: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
+    H = s.shape[1]
+    alpha = out if out is not None else torch.empty_like(s)
+    _check(lib().tg_edge_softmax_fwd(b.handle, C.c_int(H), _ptr(s), _ptr(alpha), _stream()), "tg_edge_softmax_fwd")
+    return alpha
+
+
+def edge_softmax_bwd(b: Block, alpha: torch.Tensor, dalpha: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
+    H = alpha.shape[1]
+    ds = out if out is not None else torch.empty_like(alpha)
+    _check(lib().tg_edge_softmax_bwd(b.handle, C.c_int(H), _ptr(alpha), _ptr(dalpha), _ptr(ds), _stream()), "tg_edge_softmax_bwd")
+    return ds
+
+
+def aggregate_fwd(b: Block, w: torch.Tensor | None, X: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
+    _rows(X, "X")
+    H, D = X.shape[1], X.shape[2]
+    Y = out if out is not None else torch.empty(b.R, H, D, dtype=X.dtype, device=X.device)
+    ws, _ = b.attn_workspace(H, D, X.dtype)
+    _check(lib().tg_aggregate_fwd(b.handle, C.c_int(H), C.c_int(D), C.c_int(_dt(X)), _ptr(w), _ptr(X), _ptr(Y), _ptr(ws),
+                                  C.c_size_t(ws.numel()), _stream()), "tg_aggregate_fwd")
+    return Y
+
+
+def aggregate_bwd(b: Block, w: torch.Tensor | None, X: torch.Tensor | None, dY: torch.Tensor, want_dw: bool = True):
+    _rows(dY, "dY")
+    H, D = dY.shape[1], dY.shape[2]
+    dX = torch.empty(b.U, H, D, dtype=dY.dtype, device=dY.device)
+    dw = torch.empty(b.E, H, dtype=torch.float32, device=dY.device) if (want_dw and X is not None) else None
+    _, ws = b.attn_workspace(H, D, dY.dtype)
+    _check(lib().tg_aggregate_bwd(b.handle, C.c_int(H), C.c_int(D), C.c_int(_dt(dY)), _ptr(w), _ptr(X), _ptr(dY), _ptr(dX),
+                                  _ptr(dw), _ptr(ws), C.c_size_t(ws.numel()), _stream()), "tg_aggregate_bwd")
+    return dX, dw
+
+
+def attn_fused_fwd(b: Block, Q: torch.Tensor, K: torch.Tensor, V: torch.Tensor, scale: float = 1.0, out=None):
+    _rows(Q, "Q"); _rows(K, "K"); _rows(V, "V")
+    H, D = Q.shape[1], Q.shape[2]
+    if out is None:
+        O = torch.empty_like(Q)
+        lse = torch.empty(b.R, H, dtype=torch.float32, device=Q.device)
+    else:
+        O, lse = out
+    ws, _ = b.attn_workspace(H, D, Q.dtype)
+    _check(lib().tg_attn_fused_fwd(b.handle, C.c_int(H), C.c_int(D), C.c_int(_dt(Q)), _ptr(Q), _ptr(K), _ptr(V), C.c_float(scale),
+                                   _ptr(O), _ptr(lse), _ptr(ws), C.c_size_t(ws.numel()), _stream()), "tg_attn_fused_fwd")
+    return O, lse
+
+
+def attn_fused_bwd(b: Block, Q, K, V, O, lse, dO, scale: float = 1.0, out=None):
+    for t, n in ((Q, "Q"), (K, "K"), (V, "V"), (O, "O"), (dO, "dO")):
+        _rows(t, n)
+    H, D = Q.shape[1], Q.shape[2]
+    if out is None:
+        dQ, dK, dV = torch.empty_like(Q), torch.empty_like(K), torch.empty_like(V)
+    else:
+        dQ, dK, dV = out
+    _, ws = b.attn_workspace(H, D, Q.dtype)
+    _check(lib().tg_attn_fused_bwd(b.handle, C.c_int(H), C.c_int(D), C.c_int(_dt(Q)), _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(lse),
+                                   _ptr(dO), C.c_float(scale), _ptr(dQ), _ptr(dK), _ptr(dV), _ptr(ws), C.c_size_t(ws.numel()),
+                                   _stream()), "tg_attn_fused_bwd")
+    return dQ, dK, dV

@@ -1,0 +1,132 @@
+// common.cuh -- internal declarations shared by the libfasttg translation units (sm_100a only).
+// Nothing here is shared with oracle/ (the CPU oracle is an independent program).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "fasttg.h"
+
+#if defined(__CUDA_ARCH__) && (__CUDA_ARCH__ < 1000)
+#error "libfasttg is written for sm_100a (B200) only"
+#endif
+
+// ---------------------------------------------------------------------------------------------
+// Errors
+// ---------------------------------------------------------------------------------------------
+void tg_set_error(const char* fmt, ...);
+
+#define TG_FAIL(code, ...)            \
+    do {                              \
+        tg_set_error(__VA_ARGS__);    \
+        return (code);                \
+    } while (0)
+
+#define TG_CUDA(expr)                                                                              \
+    do {                                                                                           \
+        cudaError_t _e = (expr);                                                                   \
+        if (_e != cudaSuccess) {                                                                   \
+            tg_set_error("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), __FILE__, __LINE__); \
+            return TG_ERR_CUDA;                                                                    \
+        }                                                                                          \
+    } while (0)
+
+#define TG_LAUNCH_CHECK(name)                                                                     \
+    do {                                                                                          \
+        cudaError_t _e = cudaGetLastError();                                                      \
+        if (_e != cudaSuccess) {                                                                  \
+            tg_set_error("launch of %s failed: %s", name, cudaGetErrorString(_e));                \
+            return TG_ERR_CUDA;                                                                   \
+        }                                                                                         \
+    } while (0)
+
+// ---------------------------------------------------------------------------------------------
+// Schedules.  A "side" is a CSR (rows, indptr): the destination side (rows = destinations, edges
+// in CSR order) or the source side (rows = unique source rows, edges in transposed order).
+// Rows are split into three tiers by degree:
+//   small : deg <= TG_SMALL_MAX        one sub-warp group per row
+//   warp  : deg <= TG_WARP_MAX         one warp per row
+//   cta   : larger                     one CTA per chunk of <= TG_CTA_CHUNK edges; a row with more
+//                                      than one chunk ("hub") writes fp32 partials, merged afterwards
+// ---------------------------------------------------------------------------------------------
+constexpr int TG_SMALL_MAX = 8;
+constexpr int TG_WARP_MAX = 256;
+constexpr int TG_CTA_CHUNK = 8192;
+constexpr int TG_CTA_THREADS = 256;
+constexpr int TG_CTA_WARPS = TG_CTA_THREADS / 32;
+
+struct tg_side {
+    int64_t n_rows = 0, n_edges = 0;
+    const int32_t* indptr = nullptr;
+    int32_t* order = nullptr;  // [n_rows]: small rows, then warp rows (cta rows are not listed)
+    int4* items = nullptr;     // cta items {row, begin, end, slot}; slot < 0: the row's only chunk
+    int4* hubs = nullptr;      // {row, first_slot, n_chunks, 0}
+    int32_t n_small = 0, n_warp = 0, n_items = 0, n_hubs = 0, n_slots = 0;
+    int32_t max_deg = 0;
+};
+
+struct tg_block {
+    int64_t R = 0, E = 0, U = 0;
+    const int32_t* indptr = nullptr;
+    const int32_t* kv_row = nullptr;
+    const int32_t* t_indptr = nullptr;
+    const int32_t* t_edge = nullptr;
+    const int32_t* t_dst = nullptr;
+    tg_side dst, src;
+};
+
+size_t tg_side_bytes(int64_t n_rows_bound, int64_t n_edges);
+// Builds one side's schedule in `ws` (must hold tg_side_bytes).  Synchronises the stream.
+tg_status_t tg_side_build(tg_side* s, int64_t n_rows, int64_t n_edges, const int32_t* indptr, void* ws,
+                          size_t ws_bytes, cudaStream_t stream);
+
+static inline size_t tg_align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+// ---------------------------------------------------------------------------------------------
+// Device helpers
+// ---------------------------------------------------------------------------------------------
+#ifdef __CUDACC__
+
+constexpr float TG_LOG2E = 1.4426950408889634f;
+constexpr float TG_LN2 = 0.6931471805599453f;
+
+__device__ __forceinline__ float tg_exp2(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// 16-byte read-only load (LDG.E.128.CONSTANT)
+__device__ __forceinline__ uint4 tg_ldg128(const void* p) {
+    uint4 r;
+    asm volatile("ld.global.nc.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ uint2 tg_ldg64(const void* p) {
+    uint2 r;
+    asm volatile("ld.global.nc.v2.u32 {%0,%1}, [%2];" : "=r"(r.x), "=r"(r.y) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ int tg_ldg_i32(const int32_t* p) {
+    int r;
+    asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(r) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ float tg_ldg_f32(const float* p) {
+    float r;
+    asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(r) : "l"(p));
+    return r;
+}
+
+__device__ __forceinline__ float tg_bf16lo(uint32_t x) { return __uint_as_float(x << 16); }
+__device__ __forceinline__ float tg_bf16hi(uint32_t x) { return __uint_as_float(x & 0xffff0000u); }
+// round-to-nearest-even pack of two floats into bf16x2 (lo = a, hi = b)
+__device__ __forceinline__ uint32_t tg_pack_bf16(float a, float b) {
+    uint32_t r;
+    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(b), "f"(a));
+    return r;
+}
+
+#endif  // __CUDACC__

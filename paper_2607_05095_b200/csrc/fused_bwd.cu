@@ -1,0 +1,66 @@
+// fused_bwd.cu -- tg_attn_fused_bwd ("forward and backward"; formulas DESIGN.md §2).
+// Pass 1, destination-major: delta, dQ (and the {lse2, delta} table).  Pass 2, source-major over the
+// transposed CSR: dK, dV by gather -- no float atomics, run-to-run bitwise reproducible.
+#include "dispatch.cuh"
+
+constexpr int TG_BWD_UNR = 2;
+
+struct BwdArgs {
+    const tg_block* b;
+    const void *Q, *K, *V, *O, *dO;
+    const float* lse;
+    float scale;
+    void *dQ, *dK, *dV;
+    void* ws;
+    size_t ws_bytes;
+    int H;
+    cudaStream_t stream;
+};
+
+template <class Tr>
+struct BwdFn {
+    static tg_status_t run(const BwdArgs& a) {
+        using T = typename Tr::T;
+        tg_geom g{Tr::NE, Tr::LPR};
+        const tg_attn_ws_sizes sz = tg_attn_ws(a.b, a.H, g);
+        tg_carver c(a.ws, a.ws_bytes);
+        float2* ld = static_cast<float2*>(c.take(sz.ld));
+        float* dq_part = static_cast<float*>(c.take(sz.dq_part));
+        float* dkv_part = static_cast<float*>(c.take(sz.dkv_part));
+        if (!c.ok()) TG_FAIL(TG_ERR_WORKSPACE, "fused bwd needs %zu workspace bytes", c.off);
+        {
+            using Op = Bwd1Op<Tr, TG_BWD_UNR>;
+            typename Op::Params p;
+            p.Q = static_cast<const T*>(a.Q); p.K = static_cast<const T*>(a.K); p.V = static_cast<const T*>(a.V);
+            p.O = static_cast<const T*>(a.O); p.dO = static_cast<const T*>(a.dO);
+            p.kv = a.b->kv_row; p.lse = a.lse;
+            p.dQ = static_cast<T*>(a.dQ); p.ld = ld; p.part = dq_part;
+            p.scale = a.scale; p.scale2 = a.scale * TG_LOG2E;
+            TG_TRY(tg_launch_tiers<Op>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst"));
+        }
+        {
+            using Op = Bwd2Op<Tr, TG_BWD_UNR>;
+            typename Op::Params p;
+            p.Q = static_cast<const T*>(a.Q); p.K = static_cast<const T*>(a.K); p.V = static_cast<const T*>(a.V);
+            p.dO = static_cast<const T*>(a.dO);
+            p.t_dst = a.b->t_dst; p.ld = ld;
+            p.dK = static_cast<T*>(a.dK); p.dV = static_cast<T*>(a.dV); p.part = dkv_part;
+            p.scale = a.scale; p.scale2 = a.scale * TG_LOG2E;
+            TG_TRY(tg_launch_tiers<Op>(p, a.b->src, a.stream, "tg_attn_fused_bwd/src"));
+        }
+        return TG_OK;
+    }
+};
+
+extern "C" tg_status_t tg_attn_fused_bwd(const tg_block_t* b, int H, int D, tg_dtype_t dtype, const void* Q, const void* K,
+                                         const void* V, const void* O, const float* lse, const void* dO, float scale,
+                                         void* dQ, void* dK, void* dV, void* ws, size_t ws_bytes, tg_stream_t stream) {
+    TG_CHECK_PTR(b);
+    if (!tg_shape_supported(H, D, dtype)) TG_FAIL(TG_ERR_UNSUPPORTED, "unsupported (H=%d, D=%d, dtype=%d)", H, D, (int)dtype);
+    if (b->R == 0) return TG_OK;
+    TG_CHECK_ROWS(Q); TG_CHECK_ROWS(O); TG_CHECK_ROWS(dO); TG_CHECK_ROWS(dQ); TG_CHECK_PTR(lse);
+    if (b->E > 0) { TG_CHECK_ROWS(K); TG_CHECK_ROWS(V); TG_CHECK_ROWS(dK); TG_CHECK_ROWS(dV); }
+    if (!ws) TG_FAIL(TG_ERR_WORKSPACE, "fused bwd needs a workspace (tg_attn_workspace_bytes)");
+    BwdArgs a{b, Q, K, V, O, dO, lse, scale, dQ, dK, dV, ws, ws_bytes, H, static_cast<cudaStream_t>(stream)};
+    return tg_dispatch<BwdFn>(H, D, dtype, a);
+}

@@ -1,0 +1,59 @@
+// fused_fwd.cu -- tg_attn_fused_fwd: SDDMM -> edge softmax -> alpha-weighted aggregation in one pass
+// (DESIGN.md §2, §5.3).  s and alpha never reach HBM.
+#include "dispatch.cuh"
+
+constexpr int TG_FWD_UNR = 2;
+
+struct FwdArgs {
+    const tg_block* b;
+    const void *Q, *K, *V;
+    float scale;
+    void* O;
+    float* lse;
+    void* ws;
+    cudaStream_t stream;
+};
+
+template <class Tr>
+struct FwdFn {
+    static tg_status_t run(const FwdArgs& a) {
+        using Op = FwdOp<Tr, TG_FWD_UNR>;
+        using T = typename Tr::T;
+        typename Op::Params p;
+        p.Q = static_cast<const T*>(a.Q); p.K = static_cast<const T*>(a.K); p.V = static_cast<const T*>(a.V);
+        p.kv = a.b->kv_row;
+        p.O = static_cast<T*>(a.O);
+        p.lse = a.lse;
+        p.part = static_cast<float*>(a.ws);
+        p.scale2 = a.scale * TG_LOG2E;
+        return tg_launch_tiers<Op>(p, a.b->dst, a.stream, "tg_attn_fused_fwd");
+    }
+};
+
+extern "C" tg_status_t tg_attn_workspace_bytes(const tg_block_t* b, int H, int D, tg_dtype_t dtype, size_t* fwd_bytes,
+                                               size_t* bwd_bytes) {
+    TG_CHECK_PTR(b);
+    tg_geom g;
+    TG_TRY(tg_get_geom(H, D, dtype, &g));
+    const tg_attn_ws_sizes s = tg_attn_ws(b, H, g);
+    // the unfused aggregate calls reuse these workspaces: fwd needs NE*LPR per dst slot, bwd NE*LPR per src slot
+    if (fwd_bytes) *fwd_bytes = tg_align_up(s.fwd_part) + 256;
+    if (bwd_bytes) *bwd_bytes = tg_align_up(s.ld) + tg_align_up(s.dq_part) + tg_align_up(s.dkv_part) + 256;
+    return TG_OK;
+}
+
+extern "C" tg_status_t tg_attn_fused_fwd(const tg_block_t* b, int H, int D, tg_dtype_t dtype, const void* Q, const void* K,
+                                         const void* V, float scale, void* O, float* lse, void* ws, size_t ws_bytes,
+                                         tg_stream_t stream) {
+    TG_CHECK_PTR(b);
+    if (!tg_shape_supported(H, D, dtype)) TG_FAIL(TG_ERR_UNSUPPORTED, "unsupported (H=%d, D=%d, dtype=%d)", H, D, (int)dtype);
+    if (b->R == 0) return TG_OK;
+    TG_CHECK_ROWS(Q); TG_CHECK_ROWS(O); TG_CHECK_PTR(lse);
+    if (b->E > 0) { TG_CHECK_ROWS(K); TG_CHECK_ROWS(V); }
+    tg_geom g;
+    TG_TRY(tg_get_geom(H, D, dtype, &g));
+    const tg_attn_ws_sizes s = tg_attn_ws(b, H, g);
+    if (s.fwd_part > 0 && (!ws || ws_bytes < s.fwd_part)) TG_FAIL(TG_ERR_WORKSPACE, "fused fwd needs %zu workspace bytes", s.fwd_part);
+    FwdArgs a{b, Q, K, V, scale, O, lse, ws, static_cast<cudaStream_t>(stream)};
+    return tg_dispatch<FwdFn>(H, D, dtype, a);
+}

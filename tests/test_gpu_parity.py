@@ -1,0 +1,263 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Index structures bit-exact; floating point within BASELINE.json's tolerances.
+Sizes are chosen so that every degree tier (small <= 8, warp <= 256, cta chunks of 8192, hub partial
+merge) and a ragged tail are exercised while the oracle still finishes in seconds."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2607_05095_b200 import workloads as W
+
+from gpu_util import TDT, assert_close, dev, gpu_block, host, oracle_fused, run_fused
+
+pytestmark = pytest.mark.gpu
+
+SHAPES = [(2, 50), (4, 32), (8, 16), (2, 64)]
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2607_05095_b200 import binding
+    binding.lib()
+    assert torch.cuda.is_available(), "no CUDA device: the product path has no CPU fallback"
+    return binding
+
+
+def _oblock(oracle_mod, w, dedup=None):
+    return oracle_mod.block_build(w.R, w.root_idx, w.nbr_node, w.edge_id, w.ts, w.dedup_mode if dedup is None else dedup)
+
+
+def _hub_workload(seed, H, D, dtype, n_hub_dst=2, hub_deg=20000, n_src=300, src_hub_frac=0.6, R=700, max_deg=300):
+    """Mixed block: random small/warp/cta rows + a few destination hubs (several cta chunks) + one hot source row
+    referenced by a large share of all edges (source-side hub with partial merge)."""
+    w = W.small_random(seed, R, max_deg, n_src, H, D, dtype=dtype, zero_frac=0.1)
+    r = np.random.default_rng(seed + 1000)
+    deg = np.bincount(w.root_idx, minlength=R)
+    hub_rows = r.choice(R, size=n_hub_dst, replace=False)
+    extra_root = np.repeat(hub_rows.astype(np.int32), hub_deg)
+    extra_nbr = r.integers(0, n_src, size=len(extra_root)).astype(np.int64) * 7 + 3
+    hot = r.random(len(extra_root)) < src_hub_frac
+    extra_nbr[hot] = 3                                      # node id 3 = source rank 0: the hot row
+    w.root_idx = np.concatenate([w.root_idx, extra_root]).astype(np.int32)
+    w.nbr_node = np.concatenate([w.nbr_node, extra_nbr])
+    p = r.permutation(len(w.root_idx))                      # unsorted sampler order
+    w.root_idx, w.nbr_node = w.root_idx[p], w.nbr_node[p]
+    w.edge_id = np.arange(len(p), dtype=np.int64)
+    w.ts = r.random(len(p), dtype=np.float32)
+    return w
+
+
+# ------------------------------------------------------------------------------------------------
+# index structures: bit-exact
+# ------------------------------------------------------------------------------------------------
+
+def _block_cases():
+    yield W.small_random(1, 40, 6, 12, 2, 4, shuffle=True)
+    yield W.small_random(2, 3000, 20, 500, 2, 4, shuffle=True)
+    yield W.small_random(3, 3000, 20, 500, 2, 4, shuffle=False)
+    yield W.small_random(4, 5, 3000, 3, 2, 4, shuffle=True)
+    yield W.small_random(5, 100, 3, 1, 2, 4, shuffle=True)
+    yield W.small_random(6, 2500, 700, 4000, 2, 4, shuffle=True, zero_frac=0.3)
+    yield W.config1(seed=0)
+
+
+@pytest.mark.parametrize("w", list(_block_cases()), ids=lambda w: w.name)
+@pytest.mark.parametrize("dedup", [0, 1])
+def test_block_build_bit_exact(B, oracle_mod, w, dedup):
+    ob = _oblock(oracle_mod, w, dedup)
+    gb = gpu_block(B, w, dedup)
+    assert gb.U == ob.U
+    for name in ("indptr", "perm", "kv_row", "uniq_node", "t_indptr", "t_edge", "t_dst", "eid_csr", "ts_csr"):
+        got, ref = host(getattr(gb, name)), getattr(ob, name)
+        assert got.dtype == ref.dtype and np.array_equal(got, ref), name
+    info = gb.info()
+    assert info["R"] == w.R and info["E"] == w.E and info["U"] == ob.U
+    deg = np.diff(ob.indptr)
+    assert info["dst_small"] == int((deg <= 8).sum()) and info["dst_warp"] == int(((deg > 8) & (deg <= 256)).sum())
+
+
+def test_block_build_negative_ids_and_empty(B, oracle_mod):
+    w = W.small_random(7, 50, 9, 30, 2, 4, shuffle=True)
+    w.nbr_node = w.nbr_node - 100                           # negative node ids: full 64-bit key sort
+    ob = _oblock(oracle_mod, w, 1)
+    gb = gpu_block(B, w, 1)
+    for name in ("kv_row", "uniq_node", "t_indptr", "t_edge", "t_dst"):
+        assert np.array_equal(host(getattr(gb, name)), getattr(ob, name)), name
+    e = B.block_build(3, dev(np.zeros(0, np.int32)), dev(np.zeros(0, np.int64)), None, None, 1)
+    assert e.U == 0 and host(e.indptr).tolist() == [0, 0, 0, 0] and host(e.t_indptr).tolist() == [0]
+    e0 = B.block_build(0, dev(np.zeros(0, np.int32)), dev(np.zeros(0, np.int64)), None, None, 0)
+    assert e0.U == 0 and host(e0.indptr).tolist() == [0]
+    with pytest.raises(B.FastTGError) as ei:
+        B.block_build(2, dev(np.array([0, 2], np.int32)), dev(np.array([1, 1], np.int64)), None, None, 1)
+    assert ei.value.status == 1
+
+
+# ------------------------------------------------------------------------------------------------
+# fused forward + backward
+# ------------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("H,D", SHAPES + [(1, 128), (2, 32), (4, 16), (2, 128)])
+def test_fused_small_blocks(B, oracle_mod, H, D, dtype):
+    """degrees 0..40: small + warp tiers, zero-degree rows, ragged group tails."""
+    w = W.small_random(100 + H * D, 500, 40, 120, H, D, dtype=dtype, shuffle=True, zero_frac=0.15)
+    ob = _oblock(oracle_mod, w)
+    gb = gpu_block(B, w)
+    feats = w.features(ob.U)
+    scale = 2.0
+    got = run_fused(B, gb, w, feats, scale)
+    ref = oracle_fused(oracle_mod, ob, feats, scale)
+    for n, g, r in zip(("O", "LSE", "dQ", "dK", "dV"), got, ref):
+        assert_close(n, g, r, dtype)
+    deg = np.diff(ob.indptr)
+    assert np.all(got[0][deg == 0] == 0) and np.all(got[2][deg == 0] == 0)      # zero-degree: O = dQ = 0, LSE = -inf
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("H,D", SHAPES)
+def test_fused_all_tiers_with_hubs(B, oracle_mod, H, D, dtype):
+    """cta tier, multi-chunk destination hubs (partial (m,l,acc) merge) and a hot source row (dK/dV partial merge)."""
+    w = _hub_workload(7 + H, H, D, dtype)
+    ob = _oblock(oracle_mod, w)
+    gb = gpu_block(B, w)
+    info = gb.info()
+    assert info["dst_slots"] >= 4 and info["src_slots"] >= 2 and info["dst_cta_items"] > info["dst_slots"]
+    feats = w.features(ob.U)
+    scale = float(math.sqrt(D))                                              # logits ~ N(0,1): softmax far from uniform
+    got = run_fused(B, gb, w, feats, scale)
+    ref = oracle_fused(oracle_mod, ob, feats, scale)
+    for n, g, r in zip(("O", "LSE", "dQ", "dK", "dV"), got, ref):
+        assert_close(n, g, r, dtype)
+
+
+@pytest.mark.parametrize("scale", [1.0, 1e4])
+def test_fused_degree_thresholds_and_large_logits(B, oracle_mod, scale):
+    """degrees straddling every internal threshold (8/9, 256/257, 8192/8193) and logits x 1e4 (max subtraction)."""
+    degs = [0, 1, 2, 7, 8, 9, 10, 255, 256, 257, 258, 8191, 8192, 8193, 16384, 16385]
+    H, D = 2, 64
+    root = np.repeat(np.arange(len(degs), dtype=np.int32), degs)
+    r = np.random.default_rng(5)
+    nbr = r.integers(0, 2000, size=len(root)).astype(np.int64)
+    w = W.Workload("thresholds", 98, 5, len(degs), H, D, "f32", scale, 1, root, nbr, np.arange(len(root), dtype=np.int64),
+                   r.random(len(root), dtype=np.float32))
+    ob = _oblock(oracle_mod, w)
+    gb = gpu_block(B, w)
+    feats = w.features(ob.U)
+    got = run_fused(B, gb, w, feats, scale)
+    ref = oracle_fused(oracle_mod, ob, feats, scale)
+    for n, g, r_ in zip(("O", "LSE", "dQ", "dK", "dV"), got, ref):
+        assert_close(n, g, r_, "f32")
+
+
+def test_fused_identity_rows_and_single_source(B, oracle_mod):
+    """dedup_mode 0 (per-edge K/V rows, config 1 as written) and U = 1 (all edges share one source row)."""
+    w = W.small_random(21, 300, 12, 40, 2, 50, shuffle=True, dedup_mode=0)
+    ob = _oblock(oracle_mod, w)
+    gb = gpu_block(B, w)
+    assert gb.U == w.E
+    feats = w.features(ob.U)
+    for n, g, r in zip(("O", "LSE", "dQ", "dK", "dV"), run_fused(B, gb, w, feats, 1.5), oracle_fused(oracle_mod, ob, feats, 1.5)):
+        assert_close(n, g, r, "f32")
+    w = W.small_random(22, 400, 30, 1, 4, 32, dtype="bf16", shuffle=True)
+    ob = _oblock(oracle_mod, w)
+    gb = gpu_block(B, w)
+    assert gb.U == 1
+    feats = w.features(1)
+    for n, g, r in zip(("O", "LSE", "dQ", "dK", "dV"), run_fused(B, gb, w, feats, 3.0), oracle_fused(oracle_mod, ob, feats, 3.0)):
+        assert_close(n, g, r, "bf16")
+
+
+def test_fused_bitwise_reproducible(B):
+    """no float atomics anywhere: two runs give identical bits."""
+    w = _hub_workload(3, 8, 16, "bf16")
+    gb = gpu_block(B, w)
+    feats = w.features(gb.U)
+    a = run_fused(B, gb, w, feats, 4.0)
+    b = run_fused(B, gb, w, feats, 4.0)
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y, equal_nan=True)
+
+
+# ------------------------------------------------------------------------------------------------
+# unfused operators
+# ------------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("H,D", SHAPES)
+def test_unfused_chain(B, oracle_mod, H, D, dtype):
+    w = _hub_workload(40 + H, H, D, dtype, hub_deg=9000)
+    ob = _oblock(oracle_mod, w)
+    gb = gpu_block(B, w)
+    q, k, v, do = w.features(ob.U)
+    tq, tk, tv, tdo = (dev(x, TDT[dtype]) for x in (q, k, v, do))
+    scale = float(math.sqrt(D))
+    # SDDMM
+    s_ref = oracle_mod.sddmm(ob.indptr, ob.kv_row, q, k, scale)
+    s = B.sddmm(gb, tq, tk, scale)
+    assert_close("s", host(s), s_ref, "f32" if dtype == "f32" else "bf16")
+    # ESM forward on the oracle's logits (isolates the operator)
+    s_in = dev(s_ref.astype(np.float32))
+    a_ref = oracle_mod.edge_softmax_fwd(ob.indptr, host(s_in))
+    alpha = B.edge_softmax_fwd(gb, s_in)
+    assert_close("alpha", host(alpha), a_ref, "f32")
+    sums = np.add.reduceat(host(alpha).astype(np.float64), ob.indptr[:-1][np.diff(ob.indptr) > 0], axis=0)
+    np.testing.assert_allclose(sums, 1.0, atol=2e-5)
+    # AGG forward, weighted and plain
+    a_in = dev(a_ref.astype(np.float32))
+    y_ref = oracle_mod.aggregate_fwd(ob.indptr, ob.kv_row, host(a_in), v)
+    assert_close("Y", host(B.aggregate_fwd(gb, a_in, tv)), y_ref, dtype)
+    y0_ref = oracle_mod.aggregate_fwd(ob.indptr, ob.kv_row, None, v)
+    assert_close("Y_plain", host(B.aggregate_fwd(gb, None, tv)), y0_ref, dtype)
+    # AGG backward: dX through the transposed CSR, dw
+    dx_ref, dw_ref = oracle_mod.aggregate_bwd(ob.indptr, ob.kv_row, ob.U, host(a_in), v, do)
+    dX, dw = B.aggregate_bwd(gb, a_in, tv, tdo)
+    assert_close("dX", host(dX), dx_ref, dtype)
+    assert_close("dw", host(dw), dw_ref, "f32" if dtype == "f32" else "bf16")
+    dx0_ref, _ = oracle_mod.aggregate_bwd(ob.indptr, ob.kv_row, ob.U, None, None, do, want_dw=False)
+    dX0, none = B.aggregate_bwd(gb, None, None, tdo, want_dw=False)
+    assert none is None
+    assert_close("dX_plain", host(dX0), dx0_ref, dtype)
+    # ESM backward
+    da_in = dev(dw_ref.astype(np.float32))
+    ds_ref = oracle_mod.edge_softmax_bwd(ob.indptr, host(a_in), host(da_in))
+    assert_close("ds", host(B.edge_softmax_bwd(gb, a_in, da_in)), ds_ref, "f32")
+
+
+def test_unfused_chain_equals_fused(B, oracle_mod):
+    """the DGL-style chain sddmm -> softmax -> aggregate and its backward reproduce the fused path."""
+    w = W.small_random(60, 800, 60, 200, 4, 32, shuffle=True)
+    gb = gpu_block(B, w)
+    q, k, v, do = (dev(x) for x in w.features(gb.U))
+    scale = 2.5
+    O, lse = B.attn_fused_fwd(gb, q, k, v, scale)
+    dQ, dK, dV = B.attn_fused_bwd(gb, q, k, v, O, lse, do, scale)
+    alpha = B.edge_softmax_fwd(gb, B.sddmm(gb, q, k, scale))
+    O2 = B.aggregate_fwd(gb, alpha, v)
+    dV2, dalpha = B.aggregate_bwd(gb, alpha, v, do)
+    ds = B.edge_softmax_bwd(gb, alpha, dalpha)
+    dQ2 = B.aggregate_fwd(gb, ds, k) * scale
+    dK2, _ = B.aggregate_bwd(gb, ds, None, q, want_dw=False)
+    for n, x, y in (("O", O, O2), ("dV", dV, dV2), ("dQ", dQ, dQ2), ("dK", dK, dK2 * scale)):
+        assert_close(n, host(x), host(y).astype(np.float64), "f32")
+
+
+# ------------------------------------------------------------------------------------------------
+# error behaviour of the boundary
+# ------------------------------------------------------------------------------------------------
+
+def test_boundary_errors(B):
+    w = W.small_random(70, 50, 9, 30, 2, 50, shuffle=True)
+    gb = gpu_block(B, w)
+    q, k, v, do = (dev(x) for x in w.features(gb.U))
+    with pytest.raises(B.FastTGError) as ei:                                  # (H, D) outside the compiled set
+        B.attn_fused_fwd(gb, q[:, :, :48].contiguous(), k[:, :, :48].contiguous(), v[:, :, :48].contiguous(), 1.0)
+    assert ei.value.status == 2
+    buf = torch.empty(q.numel() + 1, dtype=torch.float32, device="cuda")
+    q_mis = buf[1:].view_as(q)                                                # 4-byte offset: not 16-byte aligned
+    q_mis.copy_(q)
+    with pytest.raises(B.FastTGError) as ei:
+        B.attn_fused_fwd(gb, q_mis, k, v, 1.0)
+    assert ei.value.status == 3
+    assert B.supported(8, 16, torch.bfloat16) and not B.supported(3, 16, torch.float32)
