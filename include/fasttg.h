@@ -28,8 +28,8 @@
  *              are validated before any launch.  tg_last_error() gives thread-local detail text.
  *   Edge cases. R == 0 or E == 0 is TG_OK.  A zero-degree destination gives O = 0, LSE = -inf,
  *              dQ = 0 (reading R5).  Inputs must be finite.  Multi-edges are distinct edges.
- *   Supported (H, D): H in {1,2,4,8,16} with D in {8,16,32,50,64,128} such that H*lanes fit one warp;
- *              tg_supported() answers for a given (H, D, dtype).  Contains (2,50) (4,32) (8,16) (2,64).
+ *   Supported (H, D): (2,50) (4,32) (8,16) (2,64) (1,128) (2,32) (4,16) (2,128), each in TG_F32 and TG_BF16;
+ *              tg_supported() answers for a given (H, D, dtype); anything else is TG_ERR_UNSUPPORTED.
  *   There is no CPU fallback: without a CUDA device every compute call returns TG_ERR_CUDA.
  */
 #ifndef FASTTG_H_
@@ -172,12 +172,27 @@ TG_API tg_status_t tg_attn_fused_fwd(const tg_block_t* b, int H, int D, tg_dtype
  *   delta[v,h] = <dO[v,h,:], O[v,h,:]>;  alpha = exp(s - LSE);  dalpha = <dO[v(e)], V[r(e)]>;
  *   ds = alpha*(dalpha - delta);  dQ[v] = scale * sum_{N(v)} ds*K[r(e)];
  *   dK[u] = scale * sum_{r(e)=u} ds*Q[v(e)];  dV[u] = sum_{r(e)=u} alpha*dO[v(e)].
- * O and lse are the forward's outputs.  dQ [R,H,D]; dK,dV [U,H,D]. */
+ * O and lse are the forward's outputs.  dQ [R,H,D]; dK,dV [U,H,D].
+ * (With TG_BF16 storage delta is accumulated as sum alpha*dalpha in fp32 and O is only validated, not read:
+ *  the bf16 rounding of O would otherwise leak into dQ.) */
 TG_API tg_status_t tg_attn_fused_bwd(const tg_block_t* b, int H, int D, tg_dtype_t dtype,
                                      const void* Q, const void* K, const void* V, const void* O,
                                      const float* lse, const void* dO, float scale,
                                      void* dQ, void* dK, void* dV,
                                      void* ws, size_t ws_bytes, tg_stream_t stream);
+
+/* The two passes of tg_attn_fused_bwd as separate calls (tg_attn_fused_bwd = _dst then _src on one stream),
+ * for callers that want to time or overlap them.  _dst: destination-major, writes dQ and the internal
+ * {LSE, delta} table into `ws`; _src: source-major over the transposed CSR, reads that table from the
+ * SAME `ws`, writes dK and dV.  Arguments as in tg_attn_fused_bwd. */
+TG_API tg_status_t tg_attn_fused_bwd_dst(const tg_block_t* b, int H, int D, tg_dtype_t dtype,
+                                         const void* Q, const void* K, const void* V, const void* O,
+                                         const float* lse, const void* dO, float scale, void* dQ,
+                                         void* ws, size_t ws_bytes, tg_stream_t stream);
+TG_API tg_status_t tg_attn_fused_bwd_src(const tg_block_t* b, int H, int D, tg_dtype_t dtype,
+                                         const void* Q, const void* K, const void* V, const void* dO,
+                                         float scale, void* dK, void* dV,
+                                         void* ws, size_t ws_bytes, tg_stream_t stream);
 
 #ifdef __cplusplus
 }

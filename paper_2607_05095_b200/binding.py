@@ -24,7 +24,7 @@ EXPORTS = [
     "tg_block_workspace_bytes", "tg_block_build", "tg_sched_workspace_bytes", "tg_block_from_csr",
     "tg_block_destroy", "tg_block_info",
     "tg_sddmm", "tg_edge_softmax_fwd", "tg_edge_softmax_bwd", "tg_aggregate_fwd", "tg_aggregate_bwd",
-    "tg_attn_workspace_bytes", "tg_attn_fused_fwd", "tg_attn_fused_bwd",
+    "tg_attn_workspace_bytes", "tg_attn_fused_fwd", "tg_attn_fused_bwd", "tg_attn_fused_bwd_dst", "tg_attn_fused_bwd_src",
 ]
 
 
@@ -245,3 +245,23 @@ def attn_fused_bwd(b: Block, Q, K, V, O, lse, dO, scale: float = 1.0, out=None):
                                    _ptr(dO), C.c_float(scale), _ptr(dQ), _ptr(dK), _ptr(dV), _ptr(ws), C.c_size_t(ws.numel()),
                                    _stream()), "tg_attn_fused_bwd")
     return dQ, dK, dV
+
+
+def attn_fused_bwd_dst(b: Block, Q, K, V, O, lse, dO, scale: float, dQ):
+    """First half of attn_fused_bwd (destination-major): dQ and the internal {LSE, delta} table."""
+    H, D = Q.shape[1], Q.shape[2]
+    _, ws = b.attn_workspace(H, D, Q.dtype)
+    _check(lib().tg_attn_fused_bwd_dst(b.handle, C.c_int(H), C.c_int(D), C.c_int(_dt(Q)), _ptr(Q), _ptr(K), _ptr(V), _ptr(O),
+                                       _ptr(lse), _ptr(dO), C.c_float(scale), _ptr(dQ), _ptr(ws), C.c_size_t(ws.numel()),
+                                       _stream()), "tg_attn_fused_bwd_dst")
+    return dQ
+
+
+def attn_fused_bwd_src(b: Block, Q, K, V, dO, scale: float, dK, dV):
+    """Second half of attn_fused_bwd (source-major over the transposed CSR): dK, dV."""
+    H, D = Q.shape[1], Q.shape[2]
+    _, ws = b.attn_workspace(H, D, Q.dtype)
+    _check(lib().tg_attn_fused_bwd_src(b.handle, C.c_int(H), C.c_int(D), C.c_int(_dt(Q)), _ptr(Q), _ptr(K), _ptr(V), _ptr(dO),
+                                       C.c_float(scale), _ptr(dK), _ptr(dV), _ptr(ws), C.c_size_t(ws.numel()), _stream()),
+           "tg_attn_fused_bwd_src")
+    return dK, dV

@@ -73,7 +73,7 @@ static inline tg_attn_ws_sizes tg_attn_ws(const tg_block* b, int H, const tg_geo
     tg_attn_ws_sizes s;
     s.fwd_part = (size_t)b->dst.n_slots * (g.NE + 2) * g.LPR * sizeof(float);
     s.ld = (size_t)b->R * H * sizeof(float2);
-    s.dq_part = (size_t)b->dst.n_slots * g.NE * g.LPR * sizeof(float);
+    s.dq_part = (size_t)b->dst.n_slots * (2 * g.NE + 1) * g.LPR * sizeof(float);  // bf16: {A1, A2, d}; fp32 uses NE of it
     s.dkv_part = (size_t)b->src.n_slots * 2 * g.NE * g.LPR * sizeof(float);
     return s;
 }

@@ -19,7 +19,8 @@ struct BwdArgs {
 
 template <class Tr>
 struct BwdFn {
-    static tg_status_t run(const BwdArgs& a) {
+    // which: 1 = destination-major pass only, 2 = source-major pass only, 3 = both
+    static tg_status_t run(const BwdArgs& a, int which) {
         using T = typename Tr::T;
         tg_geom g{Tr::NE, Tr::LPR};
         const tg_attn_ws_sizes sz = tg_attn_ws(a.b, a.H, g);
@@ -28,7 +29,7 @@ struct BwdFn {
         float* dq_part = static_cast<float*>(c.take(sz.dq_part));
         float* dkv_part = static_cast<float*>(c.take(sz.dkv_part));
         if (!c.ok()) TG_FAIL(TG_ERR_WORKSPACE, "fused bwd needs %zu workspace bytes", c.off);
-        {
+        if (which & 1) {
             using Op = Bwd1Op<Tr, TG_BWD_UNR>;
             typename Op::Params p;
             p.Q = static_cast<const T*>(a.Q); p.K = static_cast<const T*>(a.K); p.V = static_cast<const T*>(a.V);
@@ -38,7 +39,7 @@ struct BwdFn {
             p.scale = a.scale; p.scale2 = a.scale * TG_LOG2E;
             TG_TRY(tg_launch_tiers<Op>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst"));
         }
-        {
+        if (which & 2) {
             using Op = Bwd2Op<Tr, TG_BWD_UNR>;
             typename Op::Params p;
             p.Q = static_cast<const T*>(a.Q); p.K = static_cast<const T*>(a.K); p.V = static_cast<const T*>(a.V);
@@ -52,15 +53,37 @@ struct BwdFn {
     }
 };
 
-extern "C" tg_status_t tg_attn_fused_bwd(const tg_block_t* b, int H, int D, tg_dtype_t dtype, const void* Q, const void* K,
-                                         const void* V, const void* O, const float* lse, const void* dO, float scale,
-                                         void* dQ, void* dK, void* dV, void* ws, size_t ws_bytes, tg_stream_t stream) {
+static tg_status_t bwd_common(const tg_block_t* b, int H, int D, tg_dtype_t dtype, const void* Q, const void* K, const void* V,
+                              const void* O, const float* lse, const void* dO, float scale, void* dQ, void* dK, void* dV,
+                              void* ws, size_t ws_bytes, tg_stream_t stream, int which) {
     TG_CHECK_PTR(b);
     if (!tg_shape_supported(H, D, dtype)) TG_FAIL(TG_ERR_UNSUPPORTED, "unsupported (H=%d, D=%d, dtype=%d)", H, D, (int)dtype);
     if (b->R == 0) return TG_OK;
-    TG_CHECK_ROWS(Q); TG_CHECK_ROWS(O); TG_CHECK_ROWS(dO); TG_CHECK_ROWS(dQ); TG_CHECK_PTR(lse);
-    if (b->E > 0) { TG_CHECK_ROWS(K); TG_CHECK_ROWS(V); TG_CHECK_ROWS(dK); TG_CHECK_ROWS(dV); }
+    TG_CHECK_ROWS(Q); TG_CHECK_ROWS(dO);
+    if (which & 1) { TG_CHECK_ROWS(O); TG_CHECK_ROWS(dQ); TG_CHECK_PTR(lse); }
+    if (b->E > 0) {
+        TG_CHECK_ROWS(K); TG_CHECK_ROWS(V);
+        if (which & 2) { TG_CHECK_ROWS(dK); TG_CHECK_ROWS(dV); }
+    }
     if (!ws) TG_FAIL(TG_ERR_WORKSPACE, "fused bwd needs a workspace (tg_attn_workspace_bytes)");
     BwdArgs a{b, Q, K, V, O, dO, lse, scale, dQ, dK, dV, ws, ws_bytes, H, static_cast<cudaStream_t>(stream)};
-    return tg_dispatch<BwdFn>(H, D, dtype, a);
+    return tg_dispatch<BwdFn>(H, D, dtype, a, which);
+}
+
+extern "C" tg_status_t tg_attn_fused_bwd(const tg_block_t* b, int H, int D, tg_dtype_t dtype, const void* Q, const void* K,
+                                         const void* V, const void* O, const float* lse, const void* dO, float scale,
+                                         void* dQ, void* dK, void* dV, void* ws, size_t ws_bytes, tg_stream_t stream) {
+    return bwd_common(b, H, D, dtype, Q, K, V, O, lse, dO, scale, dQ, dK, dV, ws, ws_bytes, stream, 3);
+}
+
+extern "C" tg_status_t tg_attn_fused_bwd_dst(const tg_block_t* b, int H, int D, tg_dtype_t dtype, const void* Q, const void* K,
+                                             const void* V, const void* O, const float* lse, const void* dO, float scale,
+                                             void* dQ, void* ws, size_t ws_bytes, tg_stream_t stream) {
+    return bwd_common(b, H, D, dtype, Q, K, V, O, lse, dO, scale, dQ, nullptr, nullptr, ws, ws_bytes, stream, 1);
+}
+
+extern "C" tg_status_t tg_attn_fused_bwd_src(const tg_block_t* b, int H, int D, tg_dtype_t dtype, const void* Q, const void* K,
+                                             const void* V, const void* dO, float scale, void* dK, void* dV, void* ws,
+                                             size_t ws_bytes, tg_stream_t stream) {
+    return bwd_common(b, H, D, dtype, Q, K, V, nullptr, nullptr, dO, scale, nullptr, dK, dV, ws, ws_bytes, stream, 2);
 }

@@ -168,3 +168,25 @@ __device__ __forceinline__ void row_axpy(float* acc, float p, const RowReg<Tr>& 
         for (int i = 0; i < Tr::NW; ++i) acc[i] = fmaf(p, __uint_as_float(r.w[i]), acc[i]);
     }
 }
+
+// acc1 += p1 * row; acc2 += p2 * row  (one widening of the row for both)
+template <class Tr>
+__device__ __forceinline__ void row_axpy2(float* acc1, float* acc2, float p1, float p2, const RowReg<Tr>& r) {
+    if constexpr (Tr::BF16) {
+#pragma unroll
+        for (int i = 0; i < Tr::NW; ++i) {
+            const float lo = tg_bf16lo(r.w[i]), hi = tg_bf16hi(r.w[i]);
+            acc1[2 * i] = fmaf(p1, lo, acc1[2 * i]);
+            acc1[2 * i + 1] = fmaf(p1, hi, acc1[2 * i + 1]);
+            acc2[2 * i] = fmaf(p2, lo, acc2[2 * i]);
+            acc2[2 * i + 1] = fmaf(p2, hi, acc2[2 * i + 1]);
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < Tr::NW; ++i) {
+            const float x = __uint_as_float(r.w[i]);
+            acc1[i] = fmaf(p1, x, acc1[i]);
+            acc2[i] = fmaf(p2, x, acc2[i]);
+        }
+    }
+}

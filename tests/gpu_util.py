@@ -27,7 +27,9 @@ def gpu_block(B, w, dedup=None):
                          w.dedup_mode if dedup is None else dedup)
 
 
-def assert_close(name, got, ref, dtype):
+def assert_close(name, got, ref, dtype, extra_atol=0.0):
+    """extra_atol (scalar or array): an additional absolute term a test derives from the arithmetic
+    (condition number of a long fp32 sum, logit-scale amplification); 0 for the BASELINE.json bound."""
     atol, rtol, nmax = TOL[dtype]
     got = np.asarray(got, dtype=np.float64)
     ref = np.asarray(ref, dtype=np.float64)
@@ -37,12 +39,13 @@ def assert_close(name, got, ref, dtype):
     inf = np.isneginf(ref)
     assert np.array_equal(np.isneginf(got), inf), f"{name}: -inf pattern differs"
     g, r = got[~inf], ref[~inf]
+    extra = np.broadcast_to(np.asarray(extra_atol, dtype=np.float64), ref.shape)[~inf]
     assert np.all(np.isfinite(g)), f"{name}: non-finite values"
     err = np.abs(g - r)
-    bad = err > atol + rtol * np.abs(r)
+    bad = err > atol + rtol * np.abs(r) + extra
     assert not bad.any(), f"{name}: {bad.sum()} of {bad.size} outside |d| <= {atol} + {rtol}|ref|; worst {err.max():.3e} at ref {r[np.argmax(err)]:.3e}"
-    if r.size and np.abs(r).max() > 0:
-        n = err.max() / np.abs(r).max()
+    if r.size and np.abs(r).max() > 100 * atol:      # a tensor that is ~0 everywhere is judged by atol alone
+        n = np.max(np.maximum(err - extra, 0.0)) / np.abs(r).max()
         assert n <= nmax, f"{name}: max error / max |ref| = {n:.3e} > {nmax}"
 
 
