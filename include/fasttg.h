@@ -69,6 +69,10 @@ typedef struct tg_block tg_block_t;
 TG_API const char* tg_status_string(tg_status_t s);
 TG_API const char* tg_last_error(void);
 TG_API int tg_version(void);
+/* Number of kernels this library has launched in the process so far (all threads, all streams):
+ * the difference across a timed region is the library's launch count for it.  Library sort launches
+ * inside tg_block_build (cub) are not counted. */
+TG_API unsigned long long tg_launch_count(void);
 /* 1 if (H, D, dtype) has a compiled kernel path, else 0. */
 TG_API int tg_supported(int H, int D, tg_dtype_t dtype);
 
@@ -119,7 +123,8 @@ TG_API tg_status_t tg_block_from_csr(int64_t R, int64_t E, int64_t U,
 TG_API tg_status_t tg_block_destroy(tg_block_t* b);
 
 /* Sizes and schedule statistics of a block (HOST outputs; any may be null).
- * stats[0..7] = dst side {n_small, n_warp, n_cta_items, n_partial_slots}, src side the same. */
+ * stats[0..7] = dst side {group-tier rows with degree <= 8, group-tier rows with degree 9..64, warp-tier
+ * chunk items (rows with degree > 64, one per <= 512 edges), partial slots of multi-chunk rows}, src side the same. */
 TG_API tg_status_t tg_block_info(const tg_block_t* b, int64_t* R, int64_t* E, int64_t* U, int64_t stats[8]);
 
 /* ------------------------------------------------------------------------------------------------

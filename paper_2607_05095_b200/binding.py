@@ -20,7 +20,7 @@ TG_F32, TG_BF16 = 0, 1
 _DTYPES = {torch.float32: TG_F32, torch.bfloat16: TG_BF16}
 
 EXPORTS = [
-    "tg_status_string", "tg_last_error", "tg_version", "tg_supported",
+    "tg_status_string", "tg_last_error", "tg_version", "tg_supported", "tg_launch_count",
     "tg_block_workspace_bytes", "tg_block_build", "tg_sched_workspace_bytes", "tg_block_from_csr",
     "tg_block_destroy", "tg_block_info",
     "tg_sddmm", "tg_edge_softmax_fwd", "tg_edge_softmax_bwd", "tg_aggregate_fwd", "tg_aggregate_bwd",
@@ -43,10 +43,16 @@ def lib() -> C.CDLL:
         L = C.CDLL(_LIB_PATH)
         L.tg_status_string.restype = C.c_char_p
         L.tg_last_error.restype = C.c_char_p
+        L.tg_launch_count.restype = C.c_ulonglong
         for name in EXPORTS:
             getattr(L, name)  # fail loudly on a missing symbol
         _lib = L
     return _lib
+
+
+def launch_count() -> int:
+    """tg_launch_count: kernels launched by the library in this process so far."""
+    return int(lib().tg_launch_count())
 
 
 def _check(st: int, where: str):
@@ -103,7 +109,7 @@ class Block:
         R, E, U = C.c_int64(), C.c_int64(), C.c_int64()
         stats = (C.c_int64 * 8)()
         _check(lib().tg_block_info(self.handle, C.byref(R), C.byref(E), C.byref(U), stats), "tg_block_info")
-        keys = ["dst_small", "dst_warp", "dst_cta_items", "dst_slots", "src_small", "src_warp", "src_cta_items", "src_slots"]
+        keys = ["dst_group_small", "dst_group_big", "dst_warp_items", "dst_slots", "src_group_small", "src_group_big", "src_warp_items", "src_slots"]
         return {"R": R.value, "E": E.value, "U": U.value, **{k: int(v) for k, v in zip(keys, stats)}}
 
     def attn_workspace(self, H: int, D: int, dtype: torch.dtype):

@@ -1,6 +1,8 @@
 // api.cu -- status strings, thread-local error text, version and capability queries.
 #include <stdarg.h>
 
+#include <atomic>
+
 #include "dispatch.cuh"
 
 static thread_local char g_err[512] = "";
@@ -13,6 +15,10 @@ void tg_set_error(const char* fmt, ...) {
 }
 
 extern "C" const char* tg_last_error(void) { return g_err; }
+
+static std::atomic<unsigned long long> g_launches{0};
+void tg_count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
+extern "C" unsigned long long tg_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 extern "C" const char* tg_status_string(tg_status_t s) {
     switch (s) {

@@ -19,52 +19,58 @@
 // ---------------------------------------------------------------------------------------------
 // Schedules
 // ---------------------------------------------------------------------------------------------
+// scan vector: [0, TG_NCLS) group-tier class counts, then warp items, partial slots, hubs
+constexpr int TG_SK = TG_NCLS + 3;
+
 struct SchedIn {
     const int32_t* indptr;
-    __device__ __forceinline__ IVec<5> operator()(int64_t i) const {
+    __device__ __forceinline__ IVec<TG_SK> operator()(int64_t i) const {
         const int deg = indptr[i + 1] - indptr[i];
-        IVec<5> x;
-        const int chunks = (deg > TG_WARP_MAX) ? (deg + TG_CTA_CHUNK - 1) / TG_CTA_CHUNK : 0;
-        x.v[0] = deg <= TG_SMALL_MAX;
-        x.v[1] = deg > TG_SMALL_MAX && deg <= TG_WARP_MAX;
-        x.v[2] = chunks;
-        x.v[3] = chunks > 1 ? chunks : 0;
-        x.v[4] = chunks > 1;
+        IVec<TG_SK> x = ivec_zero<TG_SK>();
+        if (deg <= TG_GROUP_MAX) {
+            x.v[tg_degree_class(deg)] = 1;
+        } else {
+            const int chunks = (deg + TG_CHUNK - 1) / TG_CHUNK;
+            x.v[TG_NCLS] = chunks;
+            x.v[TG_NCLS + 1] = chunks > 1 ? chunks : 0;
+            x.v[TG_NCLS + 2] = chunks > 1;
+        }
         return x;
     }
 };
 struct SchedOut {
     const int32_t* indptr;
-    int32_t* order;
+    int4* rows;
     int4* items;
     int4* hubs;
     int* max_deg;
-    __device__ __forceinline__ void operator()(int64_t i, const IVec<5>& ex, const IVec<5>& x, const IVec<5>& tot) const {
+    __device__ __forceinline__ void operator()(int64_t i, const IVec<TG_SK>& ex, const IVec<TG_SK>& x, const IVec<TG_SK>& tot) const {
         const int row = (int)i;
-        if (x.v[0]) order[ex.v[0]] = row;
-        if (x.v[1]) order[tot.v[0] + ex.v[1]] = row;
-        const int chunks = x.v[2];
-        if (chunks > 0) {
-            const int b = indptr[i], e = indptr[i + 1];
+        const int b = indptr[i], e = indptr[i + 1];
+        const int chunks = x.v[TG_NCLS];
+        if (chunks == 0) {
+            const int c = tg_degree_class(e - b);
+            int pos = ex.v[c];
+            for (int cc = c + 1; cc < TG_NCLS; ++cc) pos += tot.v[cc];  // larger classes come first
+            rows[pos] = make_int4(row, b, e, 0);
+        } else {
             const int len = (e - b + chunks - 1) / chunks;
             for (int c = 0; c < chunks; ++c) {
                 const int cb = min(b + c * len, e), ce = min(cb + len, e);
-                items[ex.v[2] + c] = make_int4(row, cb, ce, chunks > 1 ? ex.v[3] + c : -1);
+                items[ex.v[TG_NCLS] + c] = make_int4(row, cb, ce, chunks > 1 ? ex.v[TG_NCLS + 1] + c : -1);
             }
-            if (chunks > 1) hubs[ex.v[4]] = make_int4(row, ex.v[3], chunks, 0);
-            atomicMax(max_deg, e - b);
-        } else if (x.v[1]) {
-            atomicMax(max_deg, indptr[i + 1] - indptr[i]);
+            if (chunks > 1) hubs[ex.v[TG_NCLS + 2]] = make_int4(row, ex.v[TG_NCLS + 1], chunks, 0);
         }
+        if (e - b > 8) atomicMax(max_deg, e - b);
     }
 };
 
-static inline int64_t side_items_bound(int64_t n_edges) { return n_edges / TG_WARP_MAX + n_edges / TG_CTA_CHUNK + 2; }
-static inline int64_t side_hubs_bound(int64_t n_edges) { return n_edges / TG_CTA_CHUNK + 1; }
+static inline int64_t side_items_bound(int64_t n_edges) { return n_edges / TG_GROUP_MAX + 2; }
+static inline int64_t side_hubs_bound(int64_t n_edges) { return n_edges / TG_CHUNK + 1; }
 
 size_t tg_side_bytes(int64_t n_rows_bound, int64_t n_edges) {
-    return tg_align_up((size_t)(n_rows_bound + 1) * sizeof(int32_t)) + tg_align_up((size_t)side_items_bound(n_edges) * sizeof(int4)) +
-           tg_align_up((size_t)side_hubs_bound(n_edges) * sizeof(int4)) + tg_scan_bytes<5>(n_rows_bound) + 512;
+    return tg_align_up((size_t)(n_rows_bound + 1) * sizeof(int4)) + tg_align_up((size_t)side_items_bound(n_edges) * sizeof(int4)) +
+           tg_align_up((size_t)side_hubs_bound(n_edges) * sizeof(int4)) + tg_scan_bytes<TG_SK>(n_rows_bound) + 512;
 }
 
 tg_status_t tg_side_build(tg_side* s, int64_t n_rows, int64_t n_edges, const int32_t* indptr, void* ws, size_t ws_bytes,
@@ -73,20 +79,22 @@ tg_status_t tg_side_build(tg_side* s, int64_t n_rows, int64_t n_edges, const int
     s->n_rows = n_rows; s->n_edges = n_edges; s->indptr = indptr;
     if (n_rows == 0) return TG_OK;
     tg_carver c(ws, ws_bytes);
-    s->order = static_cast<int32_t*>(c.take((size_t)(n_rows + 1) * sizeof(int32_t)));
+    s->rows = static_cast<int4*>(c.take((size_t)(n_rows + 1) * sizeof(int4)));
     s->items = static_cast<int4*>(c.take((size_t)side_items_bound(n_edges) * sizeof(int4)));
     s->hubs = static_cast<int4*>(c.take((size_t)side_hubs_bound(n_edges) * sizeof(int4)));
-    void* scan_tmp = c.take(tg_scan_bytes<5>(n_rows));
-    int* totals = static_cast<int*>(c.take(256));  // IVec<5> + max_deg at [8]
+    void* scan_tmp = c.take(tg_scan_bytes<TG_SK>(n_rows));
+    int* totals = static_cast<int*>(c.take(256));  // IVec<TG_SK> + max_deg at [TG_SK]
     if (!c.ok()) TG_FAIL(TG_ERR_WORKSPACE, "schedule workspace too small: need %zu, have %zu", c.off, ws_bytes);
     TG_CUDA(cudaMemsetAsync(totals, 0, 256, stream));
     SchedIn in{indptr};
-    SchedOut out{indptr, s->order, s->items, s->hubs, totals + 8};
-    TG_TRY((tg_scan<5>(n_rows, in, out, scan_tmp, reinterpret_cast<IVec<5>*>(totals), stream)));
-    int h[9];
+    SchedOut out{indptr, s->rows, s->items, s->hubs, totals + TG_SK};
+    TG_TRY((tg_scan<TG_SK>(n_rows, in, out, scan_tmp, reinterpret_cast<IVec<TG_SK>*>(totals), stream)));
+    int h[TG_SK + 1];
     TG_CUDA(cudaMemcpyAsync(h, totals, sizeof(h), cudaMemcpyDeviceToHost, stream));
     TG_CUDA(cudaStreamSynchronize(stream));
-    s->n_small = h[0]; s->n_warp = h[1]; s->n_items = h[2]; s->n_slots = h[3]; s->n_hubs = h[4]; s->max_deg = h[8];
+    s->n_group = 0;
+    for (int k = 0; k < TG_NCLS; ++k) { s->n_cls[k] = h[k]; s->n_group += h[k]; }
+    s->n_items = h[TG_NCLS]; s->n_slots = h[TG_NCLS + 1]; s->n_hubs = h[TG_NCLS + 2]; s->max_deg = h[TG_SK];
     return TG_OK;
 }
 
@@ -402,8 +410,8 @@ extern "C" tg_status_t tg_block_info(const tg_block_t* b, int64_t* R, int64_t* E
     if (E) *E = b->E;
     if (U) *U = b->U;
     if (stats) {
-        stats[0] = b->dst.n_small; stats[1] = b->dst.n_warp; stats[2] = b->dst.n_items; stats[3] = b->dst.n_slots;
-        stats[4] = b->src.n_small; stats[5] = b->src.n_warp; stats[6] = b->src.n_items; stats[7] = b->src.n_slots;
+        stats[0] = b->dst.n_group_small(); stats[1] = b->dst.n_group_big(); stats[2] = b->dst.n_items; stats[3] = b->dst.n_slots;
+        stats[4] = b->src.n_group_small(); stats[5] = b->src.n_group_big(); stats[6] = b->src.n_items; stats[7] = b->src.n_slots;
     }
     return TG_OK;
 }

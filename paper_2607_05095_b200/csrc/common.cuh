@@ -33,8 +33,12 @@ void tg_set_error(const char* fmt, ...);
         }                                                                                          \
     } while (0)
 
+// process-wide count of kernels launched by the library (tg_launch_count)
+void tg_count_launch();
+
 #define TG_LAUNCH_CHECK(name)                                                                     \
     do {                                                                                          \
+        tg_count_launch();                                                                        \
         cudaError_t _e = cudaGetLastError();                                                      \
         if (_e != cudaSuccess) {                                                                  \
             tg_set_error("launch of %s failed: %s", name, cudaGetErrorString(_e));                \
@@ -45,26 +49,37 @@ void tg_set_error(const char* fmt, ...);
 // ---------------------------------------------------------------------------------------------
 // Schedules.  A "side" is a CSR (rows, indptr): the destination side (rows = destinations, edges
 // in CSR order) or the source side (rows = unique source rows, edges in transposed order).
-// Rows are split into three tiers by degree:
-//   small : deg <= TG_SMALL_MAX        one sub-warp group per row
-//   warp  : deg <= TG_WARP_MAX         one warp per row
-//   cta   : larger                     one CTA per chunk of <= TG_CTA_CHUNK edges; a row with more
-//                                      than one chunk ("hub") writes fp32 partials, merged afterwards
+// Rows are split into two tiers by degree:
+//   group tier: deg <= TG_GROUP_MAX    one sub-warp group per row (the K <= 10-20 common case); rows are
+//                                      bucketed into TG_NCLS power-of-two degree classes so that the
+//                                      groups of a warp run the same number of trips
+//   warp tier : larger                 one warp per chunk of <= TG_CHUNK edges; a row with more than one
+//                                      chunk ("hub") writes fp32 partials, merged by a second launch
+// Every schedule record carries {row, begin, end}: one load instead of the order -> indptr chain.
 // ---------------------------------------------------------------------------------------------
-constexpr int TG_SMALL_MAX = 8;
-constexpr int TG_WARP_MAX = 256;
-constexpr int TG_CTA_CHUNK = 8192;
+constexpr int TG_NCLS = 6;          // degree classes <=2, 3-4, 5-8, 9-16, 17-32, 33-64
+constexpr int TG_NCLS_SMALL = 3;    // classes 0..2 (deg <= 8) run in the high-occupancy kernel variant
+constexpr int TG_GROUP_MAX = 64;
+constexpr int TG_CHUNK = 512;
 constexpr int TG_CTA_THREADS = 256;
 constexpr int TG_CTA_WARPS = TG_CTA_THREADS / 32;
+
+__host__ __device__ constexpr int tg_degree_class(int deg) {
+    return deg <= 2 ? 0 : deg <= 4 ? 1 : deg <= 8 ? 2 : deg <= 16 ? 3 : deg <= 32 ? 4 : 5;
+}
 
 struct tg_side {
     int64_t n_rows = 0, n_edges = 0;
     const int32_t* indptr = nullptr;
-    int32_t* order = nullptr;  // [n_rows]: small rows, then warp rows (cta rows are not listed)
-    int4* items = nullptr;     // cta items {row, begin, end, slot}; slot < 0: the row's only chunk
+    int4* rows = nullptr;      // group tier {row, begin, end, 0}: class TG_NCLS-1 first ... class 0 last
+    int4* items = nullptr;     // warp tier {row, begin, end, slot}; slot < 0: the row's only chunk
     int4* hubs = nullptr;      // {row, first_slot, n_chunks, 0}
-    int32_t n_small = 0, n_warp = 0, n_items = 0, n_hubs = 0, n_slots = 0;
+    int32_t n_cls[TG_NCLS] = {0, 0, 0, 0, 0, 0};
+    int32_t n_group = 0, n_items = 0, n_hubs = 0, n_slots = 0;
     int32_t max_deg = 0;
+    // group-tier rows of the classes >= TG_NCLS_SMALL come first in `rows`
+    int32_t n_group_big() const { int n = 0; for (int c = TG_NCLS_SMALL; c < TG_NCLS; ++c) n += n_cls[c]; return n; }
+    int32_t n_group_small() const { return n_group - n_group_big(); }
 };
 
 struct tg_block {
@@ -122,6 +137,15 @@ __device__ __forceinline__ float tg_ldg_f32(const float* p) {
 
 __device__ __forceinline__ float tg_bf16lo(uint32_t x) { return __uint_as_float(x << 16); }
 __device__ __forceinline__ float tg_bf16hi(uint32_t x) { return __uint_as_float(x & 0xffff0000u); }
+// packed fp32 FMA (SASS FFMA2): (d0, d1) += (a0, a1) * (b0, b1); one issue slot for two FMAs.
+__device__ __forceinline__ void tg_ffma2(float& d0, float& d1, float a0, float a1, float b0, float b1) {
+    uint64_t a, b, c;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(a) : "f"(a0), "f"(a1));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(b) : "f"(b0), "f"(b1));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(c) : "f"(d0), "f"(d1));
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(c) : "l"(a), "l"(b));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(d0), "=f"(d1) : "l"(c));
+}
 // round-to-nearest-even pack of two floats into bf16x2 (lo = a, hi = b)
 __device__ __forceinline__ uint32_t tg_pack_bf16(float a, float b) {
     uint32_t r;

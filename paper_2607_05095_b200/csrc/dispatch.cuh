@@ -27,9 +27,9 @@ static inline bool tg_shape_supported(int H, int D, tg_dtype_t dtype) {
 }
 
 // per-lane geometry for workspace sizing
-struct tg_geom { int NE, LPR; };
+struct tg_geom { int NE, LPR, NHL; };
 template <class Tr> struct GeomFn {
-    static tg_status_t run(tg_geom* g) { g->NE = Tr::NE; g->LPR = Tr::LPR; return TG_OK; }
+    static tg_status_t run(tg_geom* g) { g->NE = Tr::NE; g->LPR = Tr::LPR; g->NHL = Tr::NHL; return TG_OK; }
 };
 static inline tg_status_t tg_get_geom(int H, int D, tg_dtype_t dtype, tg_geom* g) {
     return tg_dispatch<GeomFn>(H, D, dtype, g);
@@ -68,12 +68,15 @@ struct tg_carver {
     bool ok() const { return off <= cap && (base != nullptr || off == 0); }
 };
 
+// partial slots of one side: one per hub chunk plus the second-level slots of the split hub merge (tiers.cuh)
+static inline size_t tg_part_slots(const tg_side& s) { return (size_t)s.n_slots + (size_t)s.n_hubs * TG_HUB_SPLIT; }
+
 struct tg_attn_ws_sizes { size_t fwd_part, ld, dq_part, dkv_part; };
 static inline tg_attn_ws_sizes tg_attn_ws(const tg_block* b, int H, const tg_geom& g) {
     tg_attn_ws_sizes s;
-    s.fwd_part = (size_t)b->dst.n_slots * (g.NE + 2) * g.LPR * sizeof(float);
+    s.fwd_part = tg_part_slots(b->dst) * (g.NE + 2 * g.NHL) * g.LPR * sizeof(float);
     s.ld = (size_t)b->R * H * sizeof(float2);
-    s.dq_part = (size_t)b->dst.n_slots * (2 * g.NE + 1) * g.LPR * sizeof(float);  // bf16: {A1, A2, d}; fp32 uses NE of it
-    s.dkv_part = (size_t)b->src.n_slots * 2 * g.NE * g.LPR * sizeof(float);
+    s.dq_part = tg_part_slots(b->dst) * (2 * g.NE + g.NHL) * g.LPR * sizeof(float);  // bf16: {A1, A2, d}; fp32 uses NE of it
+    s.dkv_part = tg_part_slots(b->src) * 2 * g.NE * g.LPR * sizeof(float);
     return s;
 }

@@ -3,7 +3,13 @@
 // transposed CSR: dK, dV by gather -- no float atomics, run-to-run bitwise reproducible.
 #include "dispatch.cuh"
 
-constexpr int TG_BWD_UNR = 2;
+// launch policy {edges per trip, min CTAs per SM} for the pipelined and the plain kernel variants
+#ifndef TG_BWD1_POLICY
+#define TG_BWD1_POLICY 1, 2, 1, 3
+#endif
+#ifndef TG_BWD2_POLICY
+#define TG_BWD2_POLICY 1, 2, 1, 3
+#endif
 
 struct BwdArgs {
     const tg_block* b;
@@ -22,7 +28,7 @@ struct BwdFn {
     // which: 1 = destination-major pass only, 2 = source-major pass only, 3 = both
     static tg_status_t run(const BwdArgs& a, int which) {
         using T = typename Tr::T;
-        tg_geom g{Tr::NE, Tr::LPR};
+        tg_geom g{Tr::NE, Tr::LPR, Tr::NHL};
         const tg_attn_ws_sizes sz = tg_attn_ws(a.b, a.H, g);
         tg_carver c(a.ws, a.ws_bytes);
         float2* ld = static_cast<float2*>(c.take(sz.ld));
@@ -30,24 +36,24 @@ struct BwdFn {
         float* dkv_part = static_cast<float*>(c.take(sz.dkv_part));
         if (!c.ok()) TG_FAIL(TG_ERR_WORKSPACE, "fused bwd needs %zu workspace bytes", c.off);
         if (which & 1) {
-            using Op = Bwd1Op<Tr, TG_BWD_UNR>;
+            using Op = Bwd1Op<Tr>;
             typename Op::Params p;
             p.Q = static_cast<const T*>(a.Q); p.K = static_cast<const T*>(a.K); p.V = static_cast<const T*>(a.V);
             p.O = static_cast<const T*>(a.O); p.dO = static_cast<const T*>(a.dO);
             p.kv = a.b->kv_row; p.lse = a.lse;
             p.dQ = static_cast<T*>(a.dQ); p.ld = ld; p.part = dq_part;
             p.scale = a.scale; p.scale2 = a.scale * TG_LOG2E;
-            TG_TRY(tg_launch_tiers<Op>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst"));
+            TG_TRY((tg_launch_tiers<Op, TierPolicy<TG_BWD1_POLICY>>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst")));
         }
         if (which & 2) {
-            using Op = Bwd2Op<Tr, TG_BWD_UNR>;
+            using Op = Bwd2Op<Tr>;
             typename Op::Params p;
             p.Q = static_cast<const T*>(a.Q); p.K = static_cast<const T*>(a.K); p.V = static_cast<const T*>(a.V);
             p.dO = static_cast<const T*>(a.dO);
             p.t_dst = a.b->t_dst; p.ld = ld;
             p.dK = static_cast<T*>(a.dK); p.dV = static_cast<T*>(a.dV); p.part = dkv_part;
             p.scale = a.scale; p.scale2 = a.scale * TG_LOG2E;
-            TG_TRY(tg_launch_tiers<Op>(p, a.b->src, a.stream, "tg_attn_fused_bwd/src"));
+            TG_TRY((tg_launch_tiers<Op, TierPolicy<TG_BWD2_POLICY>>(p, a.b->src, a.stream, "tg_attn_fused_bwd/src")));
         }
         return TG_OK;
     }

@@ -2,7 +2,10 @@
 // (DESIGN.md §2, §5.3).  s and alpha never reach HBM.
 #include "dispatch.cuh"
 
-constexpr int TG_FWD_UNR = 2;
+// launch policy {edges per trip, min CTAs per SM} for the pipelined and the plain kernel variants
+#ifndef TG_FWD_POLICY
+#define TG_FWD_POLICY 2, 2, 2, 3
+#endif
 
 struct FwdArgs {
     const tg_block* b;
@@ -17,7 +20,7 @@ struct FwdArgs {
 template <class Tr>
 struct FwdFn {
     static tg_status_t run(const FwdArgs& a) {
-        using Op = FwdOp<Tr, TG_FWD_UNR>;
+        using Op = FwdOp<Tr>;
         using T = typename Tr::T;
         typename Op::Params p;
         p.Q = static_cast<const T*>(a.Q); p.K = static_cast<const T*>(a.K); p.V = static_cast<const T*>(a.V);
@@ -26,7 +29,7 @@ struct FwdFn {
         p.lse = a.lse;
         p.part = static_cast<float*>(a.ws);
         p.scale2 = a.scale * TG_LOG2E;
-        return tg_launch_tiers<Op>(p, a.b->dst, a.stream, "tg_attn_fused_fwd");
+        return tg_launch_tiers<Op, TierPolicy<TG_FWD_POLICY>>(p, a.b->dst, a.stream, "tg_attn_fused_fwd");
     }
 };
 

@@ -1,21 +1,30 @@
 // ops.cuh -- the row-gather operators that plug into tiers.cuh.
 //
-// All softmax arithmetic is done in the base-2 domain: s2 = s*log2(e), m2 = running max of s2,
+// All softmax arithmetic is done in the base-2 domain: s2 = s*log2(e), m2 = reference max of s2,
 // p = exp2(s2 - m2) (one MUFU.EX2 each), LSE = (m2 + log2 l) * ln 2.
+// Per-edge scalars are per-lane arrays over the lane's NHL head slots (rowops.cuh).
 #pragma once
 #include "tiers.cuh"
 
 #define TG_NEG_INF (-__int_as_float(0x7f800000))
+// "no edge seen yet" reference maximum: finite, so that (-inf) - m and m - m never give NaN
+constexpr float TG_NEG_BIG = -1.0e30f;
+// The online softmax rescales its accumulators only when a logit exceeds the reference maximum by more
+// than TG_TAU (base-2 units), so p <= 2^TG_TAU and the common trip carries no rescale at all.  The state
+// (m, l, acc) then stands for l*2^m, acc*2^m with m any reference <= true max + 0, >= true max - TG_TAU:
+// the merge and the final division are exact in the same way as with the true maximum.
+constexpr float TG_TAU = 8.0f;
 
 // -------------------------------------------------------------------------------------------------
-// Fused forward: online softmax (running max m2, sum l, weighted accumulator) + aggregation.
-// PAPER.md:225 (stable softmax, online normaliser ref [16]) + PAPER.md:215 (AGG).  State {m2, l, acc[NE]}.
+// Fused forward: online softmax (reference max m2, sum l, weighted accumulator) + aggregation.
+// PAPER.md:225 (stable softmax, online normaliser ref [16]) + PAPER.md:215 (AGG).
+// State {m2[NHL], l[NHL], acc[NE]}.
 // -------------------------------------------------------------------------------------------------
-template <class Tr_, int UNR_>
+template <class Tr_>
 struct FwdOp {
     using Tr = Tr_;
     using T = typename Tr::T;
-    static constexpr int UNR = UNR_, NS = Tr::NE + 2, NS1 = NS;
+    static constexpr int NHL = Tr::NHL, NS = Tr::NE + 2 * NHL, NS1 = NS;
     struct Params {
         const T *Q, *K, *V;
         const int32_t* kv;
@@ -24,64 +33,89 @@ struct FwdOp {
         float* part;
         float scale2;  // scale * log2(e)
     };
+    struct Buf { RowReg<Tr> k, v; };
     const Params& p;
     LanePos<Tr> lp;
     RowReg<Tr> q;
     __device__ __forceinline__ FwdOp(const Params& p_, int lig) : p(p_), lp(lig) {}
-    __device__ __forceinline__ void init_row(int row) { row_load(q, p.Q + (size_t)row * Tr::F, lp); }
-    __device__ __forceinline__ void init_state(float (&st)[NS]) {
-        st[0] = TG_NEG_INF;
-#pragma unroll
-        for (int i = 1; i < NS; ++i) st[i] = 0.f;
+    __device__ __forceinline__ const int32_t* idx_ptr() const { return p.kv; }
+    __device__ __forceinline__ void load(Buf& b, int r, int) const {
+        row_load(b.k, p.K + lp.off + (size_t)r * Tr::F, lp);
+        row_load(b.v, p.V + lp.off + (size_t)r * Tr::F, lp);
     }
-    __device__ __forceinline__ void edges(float (&st)[NS], int i0, int end, int stride, int trips) {
-        float m = st[0], l = st[1];
-        for (int t = 0; t < trips; ++t) {
-            bool ok[UNR];
-            RowReg<Tr> k[UNR], v[UNR];
+    __device__ __forceinline__ void init_row(int row) { row_load(q, p.Q + lp.off + (size_t)row * Tr::F, lp); }
+    __device__ __forceinline__ void init_state(float (&st)[NS]) {
 #pragma unroll
-            for (int u = 0; u < UNR; ++u) {
-                const int i = i0 + (t * UNR + u) * stride;
-                ok[u] = i < end;
-                const int r = tg_ldg_i32(p.kv + (ok[u] ? i : 0));
-                row_load(k[u], p.K + (size_t)r * Tr::F, lp);
-                row_load(v[u], p.V + (size_t)r * Tr::F, lp);
+        for (int j = 0; j < NHL; ++j) { st[j] = TG_NEG_BIG; st[NHL + j] = 0.f; }
+#pragma unroll
+        for (int i = 0; i < Tr::NE; ++i) st[2 * NHL + i] = 0.f;
+    }
+    template <int UNR, bool MASK>
+    __device__ __forceinline__ void compute(float (&st)[NS], const Buf (&b)[UNR], int pos0, int stride, int end) {
+        float s[UNR][NHL];
+        bool need = false;
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) {
+            row_dot_heads(q, b[u].k, lp, s[u]);
+            const bool ok = !MASK || (pos0 + u * stride < end);
+#pragma unroll
+            for (int j = 0; j < NHL; ++j) {
+                s[u][j] = ok ? s[u][j] * p.scale2 : TG_NEG_INF;
+                need |= s[u][j] > st[j] + TG_TAU;
             }
-            float s[UNR], mn = m;
-#pragma unroll
-            for (int u = 0; u < UNR; ++u) {
-                const float d = head_sum<Tr>(row_dot(q, k[u])) * p.scale2;
-                s[u] = ok[u] ? d : TG_NEG_INF;
-                mn = fmaxf(mn, s[u]);
-            }
-            const float ms = (mn == TG_NEG_INF) ? 0.f : mn;
-            const float corr = tg_exp2(m - ms);
-            l *= corr;
-#pragma unroll
-            for (int i = 0; i < Tr::NE; ++i) st[2 + i] *= corr;
-#pragma unroll
-            for (int u = 0; u < UNR; ++u) {
-                const float pu = tg_exp2(s[u] - ms);
-                l += pu;
-                row_axpy(st + 2, pu, v[u]);
-            }
-            m = mn;
         }
-        st[0] = m; st[1] = l;
+        if (__any_sync(0xffffffffu, need)) {
+            float c[NHL];
+#pragma unroll
+            for (int j = 0; j < NHL; ++j) {
+                float mn = st[j];
+#pragma unroll
+                for (int u = 0; u < UNR; ++u) mn = fmaxf(mn, s[u][j]);
+                c[j] = tg_exp2(st[j] - mn);
+                st[j] = mn;
+                st[NHL + j] *= c[j];
+            }
+            row_scale_heads(st + 2 * NHL, c, lp);
+        }
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) {
+            float pr[NHL];
+#pragma unroll
+            for (int j = 0; j < NHL; ++j) {
+                pr[j] = tg_exp2(s[u][j] - st[j]);
+                st[NHL + j] += pr[j];
+            }
+            row_axpy_heads(st + 2 * NHL, pr, b[u].v, lp);
+        }
     }
     __device__ __forceinline__ void merge(float (&a)[NS], const float (&b)[NS]) {
-        const float mn = fmaxf(a[0], b[0]);
-        const float ms = (mn == TG_NEG_INF) ? 0.f : mn;
-        const float ca = tg_exp2(a[0] - ms), cb = tg_exp2(b[0] - ms);
-        a[0] = mn;
+        float ca[NHL], cb[NHL];
 #pragma unroll
-        for (int i = 1; i < NS; ++i) a[i] = a[i] * ca + b[i] * cb;
+        for (int j = 0; j < NHL; ++j) {
+            const float mn = fmaxf(a[j], b[j]);
+            ca[j] = tg_exp2(a[j] - mn); cb[j] = tg_exp2(b[j] - mn);
+            a[j] = mn;
+            a[NHL + j] = a[NHL + j] * ca[j] + b[NHL + j] * cb[j];
+        }
+        float tmp[Tr::NE];
+#pragma unroll
+        for (int i = 0; i < Tr::NE; ++i) tmp[i] = b[2 * NHL + i];
+        row_scale_heads(a + 2 * NHL, ca, lp);
+        row_scale_heads(tmp, cb, lp);
+#pragma unroll
+        for (int i = 0; i < Tr::NE; ++i) a[2 * NHL + i] += tmp[i];
     }
     __device__ __forceinline__ void write_final(int row, float (&st)[NS], bool) {
-        const float l = st[1];
-        const float inv = l > 0.f ? 1.f / l : 0.f;
-        row_store(p.O + (size_t)row * Tr::F, lp, st + 2, inv);
-        if (lp.j == 0) p.lse[(size_t)row * Tr::H + lp.h] = (st[0] + log2f(l)) * TG_LN2;
+        float inv[NHL];
+#pragma unroll
+        for (int j = 0; j < NHL; ++j) inv[j] = st[NHL + j] > 0.f ? 1.f / st[NHL + j] : 0.f;
+        row_scale_heads(st + 2 * NHL, inv, lp);
+        row_store(p.O + (size_t)row * Tr::F, lp, st + 2 * NHL, 1.f);
+        if (lp.head_writer()) {
+#pragma unroll
+            for (int j = 0; j < NHL; ++j)
+                p.lse[(size_t)row * Tr::H + lp.head(j)] = st[NHL + j] > 0.f ? (st[j] + log2f(st[NHL + j])) * TG_LN2 : TG_NEG_INF;
+        }
     }
     __device__ __forceinline__ void write_partial(int slot, float (&st)[NS], bool) { tg_partial_store<Tr, NS>(p.part, slot, lp.lig, st); }
     __device__ __forceinline__ void load_partial(int slot, float (&st)[NS]) { tg_partial_load<Tr, NS>(p.part, slot, lp.lig, st); }
@@ -98,12 +132,13 @@ struct FwdOp {
 //     d = sum alpha*dalpha}, dQ = scale*(A1 - d*A2).  One extra axpy per edge, O is not read.
 // Also writes ld[v,h] = {lse2, delta} for the source-major pass.
 // -------------------------------------------------------------------------------------------------
-template <class Tr_, int UNR_>
+template <class Tr_>
 struct Bwd1Op {
     using Tr = Tr_;
     using T = typename Tr::T;
     static constexpr bool EDGE_DELTA = Tr::BF16;
-    static constexpr int UNR = UNR_, NS = EDGE_DELTA ? 2 * Tr::NE + 1 : Tr::NE, NS1 = NS;
+    static constexpr int NHL = Tr::NHL;
+    static constexpr int NS = EDGE_DELTA ? 2 * Tr::NE + NHL : Tr::NE, NS1 = NS;
     struct Params {
         const T *Q, *K, *V, *O, *dO;
         const int32_t* kv;
@@ -113,52 +148,60 @@ struct Bwd1Op {
         float* part;
         float scale, scale2;
     };
+    struct Buf { RowReg<Tr> k, v; };
     const Params& p;
     LanePos<Tr> lp;
     RowReg<Tr> q, g;
-    float lse2, delta;
+    float lse2[NHL], delta[NHL];
     int cur;
     __device__ __forceinline__ Bwd1Op(const Params& p_, int lig) : p(p_), lp(lig) {}
+    __device__ __forceinline__ const int32_t* idx_ptr() const { return p.kv; }
+    __device__ __forceinline__ void load(Buf& b, int r, int) const {
+        row_load(b.k, p.K + lp.off + (size_t)r * Tr::F, lp);
+        row_load(b.v, p.V + lp.off + (size_t)r * Tr::F, lp);
+    }
     __device__ __forceinline__ void init_row(int row) {
         cur = row;
-        row_load(q, p.Q + (size_t)row * Tr::F, lp);
-        row_load(g, p.dO + (size_t)row * Tr::F, lp);
-        delta = 0.f;
+        row_load(q, p.Q + lp.off + (size_t)row * Tr::F, lp);
+        row_load(g, p.dO + lp.off + (size_t)row * Tr::F, lp);
         if constexpr (!EDGE_DELTA) {
             RowReg<Tr> o;
-            row_load(o, p.O + (size_t)row * Tr::F, lp);
-            delta = head_sum<Tr>(row_dot(g, o));
+            row_load(o, p.O + lp.off + (size_t)row * Tr::F, lp);
+            row_dot_heads(g, o, lp, delta);
+        } else {
+#pragma unroll
+            for (int j = 0; j < NHL; ++j) delta[j] = 0.f;
         }
-        lse2 = tg_ldg_f32(p.lse + (size_t)row * Tr::H + lp.h) * TG_LOG2E;
+#pragma unroll
+        for (int j = 0; j < NHL; ++j) lse2[j] = tg_ldg_f32(p.lse + (size_t)row * Tr::H + lp.head(j)) * TG_LOG2E;
     }
     __device__ __forceinline__ void init_state(float (&st)[NS]) {
 #pragma unroll
         for (int i = 0; i < NS; ++i) st[i] = 0.f;
     }
-    __device__ __forceinline__ void edges(float (&st)[NS], int i0, int end, int stride, int trips) {
-        for (int t = 0; t < trips; ++t) {
-            bool ok[UNR];
-            RowReg<Tr> k[UNR], v[UNR];
+    template <int UNR, bool MASK>
+    __device__ __forceinline__ void compute(float (&st)[NS], const Buf (&b)[UNR], int pos0, int stride, int end) {
 #pragma unroll
-            for (int u = 0; u < UNR; ++u) {
-                const int i = i0 + (t * UNR + u) * stride;
-                ok[u] = i < end;
-                const int r = tg_ldg_i32(p.kv + (ok[u] ? i : 0));
-                row_load(k[u], p.K + (size_t)r * Tr::F, lp);
-                row_load(v[u], p.V + (size_t)r * Tr::F, lp);
-            }
+        for (int u = 0; u < UNR; ++u) {
+            float s2[NHL], da[NHL], a[NHL];
+            row_dot_heads(q, b[u].k, lp, s2);
+            row_dot_heads(g, b[u].v, lp, da);
+            const bool ok = !MASK || (pos0 + u * stride < end);
 #pragma unroll
-            for (int u = 0; u < UNR; ++u) {
-                const float s2 = head_sum<Tr>(row_dot(q, k[u])) * p.scale2;
-                const float da = head_sum<Tr>(row_dot(g, v[u]));
-                const float a = ok[u] ? tg_exp2(s2 - lse2) : 0.f;
-                if constexpr (EDGE_DELTA) {
-                    const float ada = a * da;
-                    st[2 * Tr::NE] += ada;
-                    row_axpy2(st, st + Tr::NE, ada, a, k[u]);
-                } else {
-                    row_axpy(st, a * (da - delta), k[u]);
+            for (int j = 0; j < NHL; ++j) a[j] = ok ? tg_exp2(fmaf(s2[j], p.scale2, -lse2[j])) : 0.f;
+            if constexpr (EDGE_DELTA) {
+                float ada[NHL];
+#pragma unroll
+                for (int j = 0; j < NHL; ++j) {
+                    ada[j] = a[j] * da[j];
+                    st[2 * Tr::NE + j] += ada[j];
                 }
+                row_axpy2_heads(st, st + Tr::NE, ada, a, b[u].k, lp);
+            } else {
+                float c[NHL];
+#pragma unroll
+                for (int j = 0; j < NHL; ++j) c[j] = a[j] * (da[j] - delta[j]);
+                row_axpy_heads(st, c, b[u].k, lp);
             }
         }
     }
@@ -168,21 +211,34 @@ struct Bwd1Op {
     }
     __device__ __forceinline__ void write_final(int row, float (&st)[NS], bool first) {
         if constexpr (EDGE_DELTA) {
-            const float d = st[2 * Tr::NE];
+            float d[NHL];
 #pragma unroll
-            for (int i = 0; i < Tr::NE; ++i) st[i] = fmaf(-d, st[Tr::NE + i], st[i]);
+            for (int j = 0; j < NHL; ++j) d[j] = st[2 * Tr::NE + j];
+            row_fnma_heads(st, d, st + Tr::NE, lp);
             row_store(p.dQ + (size_t)row * Tr::F, lp, st, p.scale);
             // `first` is false only in the hub merge, which owns the row's delta
-            if (lp.j == 0) p.ld[(size_t)row * Tr::H + lp.h] = make_float2(tg_ldg_f32(p.lse + (size_t)row * Tr::H + lp.h) * TG_LOG2E, d);
+            if (lp.head_writer()) {
+#pragma unroll
+                for (int j = 0; j < NHL; ++j) {
+                    const size_t o = (size_t)row * Tr::H + lp.head(j);
+                    p.ld[o] = make_float2(tg_ldg_f32(p.lse + o) * TG_LOG2E, d[j]);
+                }
+            }
         } else {
             row_store(p.dQ + (size_t)row * Tr::F, lp, st, p.scale);
-            if (first && lp.j == 0) p.ld[(size_t)cur * Tr::H + lp.h] = make_float2(lse2, delta);
+            if (first) write_ld();
+        }
+    }
+    __device__ __forceinline__ void write_ld() {
+        if (lp.head_writer()) {
+#pragma unroll
+            for (int j = 0; j < NHL; ++j) p.ld[(size_t)cur * Tr::H + lp.head(j)] = make_float2(lse2[j], delta[j]);
         }
     }
     __device__ __forceinline__ void write_partial(int slot, float (&st)[NS], bool first) {
         tg_partial_store<Tr, NS>(p.part, slot, lp.lig, st);
         if constexpr (!EDGE_DELTA) {
-            if (first && lp.j == 0) p.ld[(size_t)cur * Tr::H + lp.h] = make_float2(lse2, delta);
+            if (first) write_ld();
         }
     }
     __device__ __forceinline__ void load_partial(int slot, float (&st)[NS]) { tg_partial_load<Tr, NS>(p.part, slot, lp.lig, st); }
@@ -192,11 +248,11 @@ struct Bwd1Op {
 // Fused backward, source-major pass over the transposed CSR: dK, dV gathered, no float atomics.
 // State {dk[NE], dv[NE]}.  Row u keeps K[u], V[u]; each transposed edge gathers Q[v], dO[v], ld[v].
 // -------------------------------------------------------------------------------------------------
-template <class Tr_, int UNR_>
+template <class Tr_>
 struct Bwd2Op {
     using Tr = Tr_;
     using T = typename Tr::T;
-    static constexpr int UNR = UNR_, NS = 2 * Tr::NE, NS1 = NS;
+    static constexpr int NHL = Tr::NHL, NS = 2 * Tr::NE, NS1 = NS;
     struct Params {
         const T *Q, *K, *V, *dO;
         const int32_t* t_dst;
@@ -205,40 +261,41 @@ struct Bwd2Op {
         float* part;
         float scale, scale2;
     };
+    struct Buf { RowReg<Tr> q, g; float2 x[NHL]; };
     const Params& p;
     LanePos<Tr> lp;
     RowReg<Tr> k, v;
     __device__ __forceinline__ Bwd2Op(const Params& p_, int lig) : p(p_), lp(lig) {}
+    __device__ __forceinline__ const int32_t* idx_ptr() const { return p.t_dst; }
+    __device__ __forceinline__ void load(Buf& b, int r, int) const {
+        row_load(b.q, p.Q + lp.off + (size_t)r * Tr::F, lp);
+        row_load(b.g, p.dO + lp.off + (size_t)r * Tr::F, lp);
+#pragma unroll
+        for (int j = 0; j < NHL; ++j) b.x[j] = __ldg(p.ld + (size_t)r * Tr::H + lp.head(j));
+    }
     __device__ __forceinline__ void init_row(int row) {
-        row_load(k, p.K + (size_t)row * Tr::F, lp);
-        row_load(v, p.V + (size_t)row * Tr::F, lp);
+        row_load(k, p.K + lp.off + (size_t)row * Tr::F, lp);
+        row_load(v, p.V + lp.off + (size_t)row * Tr::F, lp);
     }
     __device__ __forceinline__ void init_state(float (&st)[NS]) {
 #pragma unroll
         for (int i = 0; i < NS; ++i) st[i] = 0.f;
     }
-    __device__ __forceinline__ void edges(float (&st)[NS], int i0, int end, int stride, int trips) {
-        for (int t = 0; t < trips; ++t) {
-            bool ok[UNR];
-            RowReg<Tr> q[UNR], g[UNR];
-            float2 x[UNR];
+    template <int UNR, bool MASK>
+    __device__ __forceinline__ void compute(float (&st)[NS], const Buf (&b)[UNR], int pos0, int stride, int end) {
 #pragma unroll
-            for (int u = 0; u < UNR; ++u) {
-                const int i = i0 + (t * UNR + u) * stride;
-                ok[u] = i < end;
-                const int r = tg_ldg_i32(p.t_dst + (ok[u] ? i : 0));
-                row_load(q[u], p.Q + (size_t)r * Tr::F, lp);
-                row_load(g[u], p.dO + (size_t)r * Tr::F, lp);
-                x[u] = __ldg(p.ld + (size_t)r * Tr::H + lp.h);
-            }
+        for (int u = 0; u < UNR; ++u) {
+            float s2[NHL], da[NHL], a[NHL], c[NHL];
+            row_dot_heads(b[u].q, k, lp, s2);
+            row_dot_heads(b[u].g, v, lp, da);
+            const bool ok = !MASK || (pos0 + u * stride < end);
 #pragma unroll
-            for (int u = 0; u < UNR; ++u) {
-                const float s2 = head_sum<Tr>(row_dot(q[u], k)) * p.scale2;
-                const float da = head_sum<Tr>(row_dot(g[u], v));
-                const float a = ok[u] ? tg_exp2(s2 - x[u].x) : 0.f;
-                row_axpy(st, a * (da - x[u].y), q[u]);
-                row_axpy(st + Tr::NE, a, g[u]);
+            for (int j = 0; j < NHL; ++j) {
+                a[j] = ok ? tg_exp2(fmaf(s2[j], p.scale2, -b[u].x[j].x)) : 0.f;
+                c[j] = a[j] * (da[j] - b[u].x[j].y);
             }
+            row_axpy_heads(st, c, b[u].q, lp);
+            row_axpy_heads(st + Tr::NE, a, b[u].g, lp);
         }
     }
     __device__ __forceinline__ void merge(float (&a)[NS], const float (&b)[NS]) {
@@ -256,39 +313,36 @@ struct Bwd2Op {
 // -------------------------------------------------------------------------------------------------
 // SDDMM: s[e,h] = scale * <A[row], B[idx[e]]> over one CSR side.  No state.
 // -------------------------------------------------------------------------------------------------
-template <class Tr_, int UNR_>
+template <class Tr_>
 struct SddmmOp {
     using Tr = Tr_;
     using T = typename Tr::T;
-    static constexpr int UNR = UNR_, NS = 0, NS1 = 1;
+    static constexpr int NHL = Tr::NHL, NS = 0, NS1 = 1;
     struct Params {
         const T *A, *B;
         const int32_t* idx;
         float* s;
         float scale;
     };
+    struct Buf { RowReg<Tr> b; };
     const Params& p;
     LanePos<Tr> lp;
     RowReg<Tr> a;
     __device__ __forceinline__ SddmmOp(const Params& p_, int lig) : p(p_), lp(lig) {}
-    __device__ __forceinline__ void init_row(int row) { row_load(a, p.A + (size_t)row * Tr::F, lp); }
+    __device__ __forceinline__ const int32_t* idx_ptr() const { return p.idx; }
+    __device__ __forceinline__ void load(Buf& b, int r, int) const { row_load(b.b, p.B + lp.off + (size_t)r * Tr::F, lp); }
+    __device__ __forceinline__ void init_row(int row) { row_load(a, p.A + lp.off + (size_t)row * Tr::F, lp); }
     __device__ __forceinline__ void init_state(float (&)[1]) {}
-    __device__ __forceinline__ void edges(float (&)[1], int i0, int end, int stride, int trips) {
-        for (int t = 0; t < trips; ++t) {
-            bool ok[UNR];
-            int e[UNR];
-            RowReg<Tr> b[UNR];
+    template <int UNR, bool MASK>
+    __device__ __forceinline__ void compute(float (&)[1], const Buf (&b)[UNR], int pos0, int stride, int end) {
 #pragma unroll
-            for (int u = 0; u < UNR; ++u) {
-                e[u] = i0 + (t * UNR + u) * stride;
-                ok[u] = e[u] < end;
-                const int r = tg_ldg_i32(p.idx + (ok[u] ? e[u] : 0));
-                row_load(b[u], p.B + (size_t)r * Tr::F, lp);
-            }
+        for (int u = 0; u < UNR; ++u) {
+            float d[NHL];
+            row_dot_heads(a, b[u].b, lp, d);
+            const int e = pos0 + u * stride;
+            if ((!MASK || e < end) && lp.head_writer()) {
 #pragma unroll
-            for (int u = 0; u < UNR; ++u) {
-                const float d = head_sum<Tr>(row_dot(a, b[u])) * p.scale;
-                if (ok[u] && lp.j == 0) p.s[(size_t)e[u] * Tr::H + lp.h] = d;
+                for (int j = 0; j < NHL; ++j) p.s[(size_t)e * Tr::H + lp.head(j)] = d[j] * p.scale;
             }
         }
     }
@@ -303,11 +357,11 @@ struct SddmmOp {
 // w == NULL: the paper's plain neighbour sum.  Forward uses (kv_row, positions),
 // backward uses the transposed side (t_dst rows of dY, weights looked up through t_edge).
 // -------------------------------------------------------------------------------------------------
-template <class Tr_, int UNR_>
+template <class Tr_>
 struct AggOp {
     using Tr = Tr_;
     using T = typename Tr::T;
-    static constexpr int UNR = UNR_, NS = Tr::NE, NS1 = NS;
+    static constexpr int NHL = Tr::NHL, NS = Tr::NE, NS1 = NS;
     struct Params {
         const T* X;
         const int32_t* idx;
@@ -316,34 +370,36 @@ struct AggOp {
         T* Y;
         float* part;
     };
+    struct Buf { RowReg<Tr> x; float w[NHL]; };
     const Params& p;
     LanePos<Tr> lp;
     __device__ __forceinline__ AggOp(const Params& p_, int lig) : p(p_), lp(lig) {}
+    __device__ __forceinline__ const int32_t* idx_ptr() const { return p.idx; }
+    __device__ __forceinline__ void load(Buf& b, int r, int pos) const {
+        row_load(b.x, p.X + lp.off + (size_t)r * Tr::F, lp);
+        if (p.w) {
+            const int we = p.widx ? tg_ldg_i32(p.widx + pos) : pos;
+#pragma unroll
+            for (int j = 0; j < NHL; ++j) b.w[j] = tg_ldg_f32(p.w + (size_t)we * Tr::H + lp.head(j));
+        } else {
+#pragma unroll
+            for (int j = 0; j < NHL; ++j) b.w[j] = 1.f;
+        }
+    }
     __device__ __forceinline__ void init_row(int) {}
     __device__ __forceinline__ void init_state(float (&st)[NS]) {
 #pragma unroll
         for (int i = 0; i < NS; ++i) st[i] = 0.f;
     }
-    __device__ __forceinline__ void edges(float (&st)[NS], int i0, int end, int stride, int trips) {
-        for (int t = 0; t < trips; ++t) {
-            float wv[UNR];
-            RowReg<Tr> x[UNR];
+    template <int UNR, bool MASK>
+    __device__ __forceinline__ void compute(float (&st)[NS], const Buf (&b)[UNR], int pos0, int stride, int end) {
 #pragma unroll
-            for (int u = 0; u < UNR; ++u) {
-                const int i = i0 + (t * UNR + u) * stride;
-                const bool ok = i < end;
-                const int ii = ok ? i : 0;
-                const int r = tg_ldg_i32(p.idx + ii);
-                row_load(x[u], p.X + (size_t)r * Tr::F, lp);
-                float wgt = 1.f;
-                if (p.w) {
-                    const int we = p.widx ? tg_ldg_i32(p.widx + ii) : ii;
-                    wgt = tg_ldg_f32(p.w + (size_t)we * Tr::H + lp.h);
-                }
-                wv[u] = ok ? wgt : 0.f;
-            }
+        for (int u = 0; u < UNR; ++u) {
+            const bool ok = !MASK || (pos0 + u * stride < end);
+            float w[NHL];
 #pragma unroll
-            for (int u = 0; u < UNR; ++u) row_axpy(st, wv[u], x[u]);
+            for (int j = 0; j < NHL; ++j) w[j] = ok ? b[u].w[j] : 0.f;
+            row_axpy_heads(st, w, b[u].x, lp);
         }
     }
     __device__ __forceinline__ void merge(float (&a)[NS], const float (&b)[NS]) {

@@ -1,10 +1,10 @@
 // softmax.cu -- tg_edge_softmax_fwd / tg_edge_softmax_bwd on [E, H] float32 edge tensors.
 // ESM: max reduction, sum reduction, element-wise division per destination; backward
 // ds = alpha*(dalpha - sum alpha*dalpha).  Tiers follow the destination-side schedule:
-//   small rows: one thread per (row, head) looping over the row's edges -- the paper's CSR "thread-loop"
-//               partitioning, which keeps every lane busy at degree <= 8;
-//   warp rows : one warp per row, lanes stride over the flat (edge, head) range, shuffle reduction;
-//   cta rows  : one CTA per row (launched on the row's first chunk item), shared-memory reduction.
+//   deg <= 8  : one thread per (row, head) looping over the row's edges -- the paper's CSR "thread-loop"
+//               partitioning, which keeps every lane busy at small degree;
+//   deg <= 64 : one warp per row, lanes stride over the flat (edge, head) range, shuffle reduction;
+//   larger    : one CTA per row (launched on the row's first chunk item), shared-memory reduction.
 // H must be a power of two <= 16 so that a lane / thread keeps one head for all its elements.
 #include "dispatch.cuh"
 
@@ -39,14 +39,16 @@ __device__ __forceinline__ float esm_cta_reduce(float x, int H, float* sm, int w
     return r;
 }
 
+// tier: 0 = warp-tier rows (one CTA per row, launched on every chunk item, only the first one works),
+//       1 = group-tier rows of the classes > 8 (one warp per row), 2 = classes <= 8 (one thread per (row, head))
 template <bool BWD>
-__global__ void __launch_bounds__(TG_CTA_THREADS) tg_esm_kernel(EsmArgs<BWD> a, SideDev sd, int H, int nb_warp) {
+__global__ void __launch_bounds__(TG_CTA_THREADS) tg_esm_kernel(EsmArgs<BWD> a, const int4* __restrict__ recs,
+                                                                const int32_t* __restrict__ indptr, int n, int H, int tier) {
     __shared__ float sm[TG_CTA_WARPS * 16];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    int bid = blockIdx.x;
-    if (bid < sd.n_items) {
-        const int4 it = sd.items[bid];
-        const int b = sd.indptr[it.x], e = sd.indptr[it.x + 1];
+    if (tier == 0) {
+        const int4 it = recs[blockIdx.x];
+        const int b = indptr[it.x], e = indptr[it.x + 1];
         if (it.y != b) return;  // only the row's first chunk item works (CTA-uniform)
         const size_t lo = (size_t)b * H, hi = (size_t)e * H;
         if (!BWD) {
@@ -64,11 +66,11 @@ __global__ void __launch_bounds__(TG_CTA_THREADS) tg_esm_kernel(EsmArgs<BWD> a, 
             d = esm_cta_reduce<false>(d, H, sm, warp, lane);
             for (size_t i = lo + threadIdx.x; i < hi; i += TG_CTA_THREADS) a.out[i] = a.a[i] * (a.b[i] - d);
         }
-    } else if ((bid -= sd.n_items) < nb_warp) {
-        const int idx = bid * TG_CTA_WARPS + warp;
-        if (idx >= sd.n_warp) return;
-        const int row = sd.order[sd.n_small + idx];
-        const size_t lo = (size_t)sd.indptr[row] * H, hi = (size_t)sd.indptr[row + 1] * H;
+    } else if (tier == 1) {
+        const int idx = blockIdx.x * TG_CTA_WARPS + warp;
+        if (idx >= n) return;
+        const int4 it = recs[idx];
+        const size_t lo = (size_t)it.y * H, hi = (size_t)it.z * H;
         if (!BWD) {
             float m = TG_NEG_INF;
             for (size_t i = lo + lane; i < hi; i += 32) m = fmaxf(m, a.a[i]);
@@ -85,13 +87,12 @@ __global__ void __launch_bounds__(TG_CTA_THREADS) tg_esm_kernel(EsmArgs<BWD> a, 
             for (size_t i = lo + lane; i < hi; i += 32) a.out[i] = a.a[i] * (a.b[i] - d);
         }
     } else {
-        bid -= nb_warp;
         const int rows_per_cta = TG_CTA_THREADS / H;
-        const int idx = bid * rows_per_cta + threadIdx.x / H;
+        const int idx = blockIdx.x * rows_per_cta + threadIdx.x / H;
         const int h = threadIdx.x % H;
-        if (idx >= sd.n_small) return;
-        const int row = sd.order[idx];
-        const int b = sd.indptr[row], e = sd.indptr[row + 1];
+        if (idx >= n) return;
+        const int4 it = recs[idx];
+        const int b = it.y, e = it.z;
         if (!BWD) {
             float m = TG_NEG_INF, l = 0.f;
             for (int i = b; i < e; ++i) m = fmaxf(m, a.a[(size_t)i * H + h]);
@@ -112,14 +113,19 @@ static tg_status_t esm_launch(const tg_block* b, int H, const float* x, const fl
     if (H < 1 || H > 16 || (H & (H - 1)) != 0) TG_FAIL(TG_ERR_UNSUPPORTED, "%s: H=%d must be a power of two <= 16", name, H);
     if (b->E == 0) return TG_OK;
     const tg_side& s = b->dst;
-    SideDev sd = tg_side_dev(s);
-    const int nb_warp = (s.n_warp + TG_CTA_WARPS - 1) / TG_CTA_WARPS;
-    const int rpc = TG_CTA_THREADS / H;
-    const int nb_small = (s.n_small + rpc - 1) / rpc;
-    const long long grid = (long long)s.n_items + nb_warp + nb_small;
     EsmArgs<BWD> a{x, y, out};
-    if (grid > 0) {
-        tg_esm_kernel<BWD><<<(unsigned)grid, TG_CTA_THREADS, 0, stream>>>(a, sd, H, nb_warp);
+    if (s.n_items > 0) {
+        tg_esm_kernel<BWD><<<(unsigned)s.n_items, TG_CTA_THREADS, 0, stream>>>(a, s.items, s.indptr, s.n_items, H, 0);
+        TG_LAUNCH_CHECK(name);
+    }
+    const int n_big = s.n_group_big(), n_small = s.n_group_small();
+    if (n_big > 0) {
+        tg_esm_kernel<BWD><<<(unsigned)((n_big + TG_CTA_WARPS - 1) / TG_CTA_WARPS), TG_CTA_THREADS, 0, stream>>>(a, s.rows, s.indptr, n_big, H, 1);
+        TG_LAUNCH_CHECK(name);
+    }
+    if (n_small > 0) {
+        const int rpc = TG_CTA_THREADS / H;
+        tg_esm_kernel<BWD><<<(unsigned)((n_small + rpc - 1) / rpc), TG_CTA_THREADS, 0, stream>>>(a, s.rows + n_big, s.indptr, n_small, H, 2);
         TG_LAUNCH_CHECK(name);
     }
     return TG_OK;

@@ -1,35 +1,25 @@
 // tiers.cuh -- the degree-tiered driver shared by every row-gather operator.
 //
-// One launch covers a whole CSR side.  blockIdx selects the tier, largest work first:
-//   [0, n_items)              cta tier  : one CTA per chunk (<= TG_CTA_CHUNK edges) of a large row; the 8
-//                                         warps take contiguous sub-ranges, groups stride inside them,
-//                                         states are merged by shuffles, then through shared memory;
-//                                         a hub (row with several chunks) writes an fp32 partial
-//   [.., + ceil(n_warp/8))    warp tier : one warp per row, its G groups stride over the row's edges
-//   [.., + ceil(n_small/8G))  small tier: one group per row (deg <= TG_SMALL_MAX, the K<=10 common case)
-// A second launch (tg_hub_kernel) merges the partials of each hub.
+// A CSR side is covered by up to four launches (largest work first):
+//   tg_warp_kernel   warp tier : one warp per chunk (<= TG_CHUNK edges) of a large row; its G groups stride
+//                                over the chunk's edges, states are merged by shuffles; a hub (row with
+//                                several chunks) writes an fp32 partial per chunk
+//   tg_hub_kernel    folds each hub's partials (two levels when a hub has more than TG_HUB_DIRECT chunks)
+//   tg_group_kernel  group tier: one group per row, degree classes 9..TG_GROUP_MAX (pipelined edge loop)
+//   tg_group_kernel  group tier: degree classes <= 8 (plain edge loop, small register budget so that more
+//                                rows are in flight: these rows are pure latency chains)
+// Rows of one class are contiguous in the schedule, so the groups of a warp run the same number of trips.
 //
 // An operator Op supplies: Tr (RowTraits), NS (fp32 state words per lane), Params, and
-//   init_row(row), init_state(st), edges(st, i0, end, stride, trips), merge(a, b),
+//   idx_ptr()                     the per-edge row index array of this side (kv_row or t_dst)
+//   Buf, load(buf, r, pos)        the gathered operands of one edge (row index r, edge position pos)
+//   compute<U, MASK>(st, buf[U], pos0, stride, end)   fold U edges pos0 + u*stride into st; MASK: edges
+//                                                      at positions >= end are ignored
+//   init_row(row), init_state(st), merge(a, b),
 //   write_final(row, st, first), write_partial(slot, st, first), load_partial(slot, st)
-// `trips` is warp-uniform so that the shuffles inside edges() are executed by all 32 lanes.
+// Every warp-wide call (compute, merge) is reached by all 32 lanes with warp-uniform trip counts.
 #pragma once
 #include "rowops.cuh"
-
-struct SideDev {
-    const int32_t* indptr;
-    const int32_t* order;
-    const int4* items;
-    const int4* hubs;
-    int n_small, n_warp, n_items, n_hubs;
-};
-
-static inline SideDev tg_side_dev(const tg_side& s) {
-    SideDev d;
-    d.indptr = s.indptr; d.order = s.order; d.items = s.items; d.hubs = s.hubs;
-    d.n_small = s.n_small; d.n_warp = s.n_warp; d.n_items = s.n_items; d.n_hubs = s.n_hubs;
-    return d;
-}
 
 template <class Op>
 __device__ __forceinline__ void tg_warp_merge(Op& op, float (&st)[Op::NS1]) {
@@ -66,77 +56,158 @@ __device__ __forceinline__ void tg_cta_merge(Op& op, float (&st)[Op::NS1], float
     }
 }
 
-template <class Op>
-__global__ void __launch_bounds__(TG_CTA_THREADS) tg_tier_kernel(typename Op::Params p, SideDev sd, int nb_warp) {
-    using Tr = typename Op::Tr;
-    __shared__ float sm[Op::NS > 0 ? TG_CTA_WARPS * Tr::LPR * Op::NS : 1];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int g = lane / Tr::LPR;
-    Op op(p, lane % Tr::LPR);
-    float st[Op::NS1];
-    int bid = blockIdx.x;
-    if (bid < sd.n_items) {
-        const int4 it = sd.items[bid];
-        const int n = it.z - it.y;
-        const int per = (n + TG_CTA_WARPS - 1) / TG_CTA_WARPS;
-        const int wb = min(it.y + warp * per, it.z), we = min(wb + per, it.z);
-        op.init_row(it.x);
-        op.init_state(st);
-        const int trips = (we - wb + Tr::G * Op::UNR - 1) / (Tr::G * Op::UNR);
-        op.edges(st, wb + g, we, Tr::G, trips);
-        tg_warp_merge(op, st);
-        tg_cta_merge(op, st, sm, warp, lane);
-        if (warp == 0 && lane < Tr::LPR) {
-            const bool first = (it.y == sd.indptr[it.x]);
-            if (it.w < 0) op.write_final(it.x, st, first);
-            else op.write_partial(it.w, st, first);
-        }
-    } else if ((bid -= sd.n_items) < nb_warp) {
-        const int idx = bid * TG_CTA_WARPS + warp;
-        if (idx >= sd.n_warp) return;
-        const int row = sd.order[sd.n_small + idx];
-        const int b = sd.indptr[row], e = sd.indptr[row + 1];
-        op.init_row(row);
-        op.init_state(st);
-        const int trips = (e - b + Tr::G * Op::UNR - 1) / (Tr::G * Op::UNR);
-        op.edges(st, b + g, e, Tr::G, trips);
-        tg_warp_merge(op, st);
-        if (lane < Tr::LPR) op.write_final(row, st, true);
-    } else {
-        bid -= nb_warp;
-        const int idx = (bid * TG_CTA_WARPS + warp) * Tr::G + g;
-        const bool active = idx < sd.n_small;
-        const int row = active ? sd.order[idx] : 0;
-        int b = 0, e = 0;
-        if (active) { b = sd.indptr[row]; e = sd.indptr[row + 1]; }
-        op.init_row(row);  // all lanes: init_row may shuffle (an idle group re-reads row 0)
-        op.init_state(st);
-        const int trips = __reduce_max_sync(0xffffffffu, (e - b + Op::UNR - 1) / Op::UNR);
-        op.edges(st, b, e, 1, trips);
-        if (active) op.write_final(row, st, true);
+// Plain edge loop of one group: edges pos = i0 + n*stride < end, U per trip, all loads of a trip issued
+// before its arithmetic.  Latency is hidden by the other warps (small register budget).
+template <int U, class Op>
+__device__ __forceinline__ void tg_run_edges_plain(Op& op, float (&st)[Op::NS1], int i0, int end, int stride, int trips) {
+    if (trips <= 0) return;
+    const int32_t* __restrict__ idx = op.idx_ptr();
+    const int last = max(end - 1, 0);
+    int pos = i0;
+    for (int t = 0; t < trips; ++t) {
+        typename Op::Buf A[U];
+        int r[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) r[u] = tg_ldg_i32(idx + min(pos + u * stride, last));
+#pragma unroll
+        for (int u = 0; u < U; ++u) op.load(A[u], r[u], min(pos + u * stride, last));
+        op.template compute<U, true>(st, A, pos, stride, end);
+        pos += U * stride;
     }
 }
 
-// One CTA per hub: every (warp, group) folds a strided subset of the hub's partial slots.
+// Software-pipelined edge loop with two register buffers: while trip t is computed the rows of trip t+1
+// are in flight and the row indices of trip t+2 are being fetched, so a warp exposes the gather latency
+// once per loop, not once per trip.  Positions past `end` are clamped for the loads (a valid row is fetched
+// again) and masked in compute().  `full_until`: trips whose first position is below it need no mask
+// (warp-uniform; pass i0 to mask everything).
+template <int U, class Op>
+__device__ __forceinline__ void tg_run_edges_pipe(Op& op, float (&st)[Op::NS1], int i0, int end, int stride, int trips,
+                                                  int full_until) {
+    if (trips <= 0) return;
+    const int32_t* __restrict__ idx = op.idx_ptr();
+    const int last = max(end - 1, 0);
+    typename Op::Buf A[U], B[U];
+    int ra[U], rb[U];
+    const int step = U * stride;
+    int pos = i0;  // first position of the trip being computed
+#pragma unroll
+    for (int u = 0; u < U; ++u) ra[u] = tg_ldg_i32(idx + min(pos + u * stride, last));
+#pragma unroll
+    for (int u = 0; u < U; ++u) op.load(A[u], ra[u], min(pos + u * stride, last));
+#pragma unroll
+    for (int u = 0; u < U; ++u) rb[u] = tg_ldg_i32(idx + min(pos + step + u * stride, last));
+    for (int t = 0; t < trips; t += 2) {
+        if (t + 1 < trips) {
+#pragma unroll
+            for (int u = 0; u < U; ++u) op.load(B[u], rb[u], min(pos + step + u * stride, last));
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) ra[u] = tg_ldg_i32(idx + min(pos + 2 * step + u * stride, last));
+        if (pos < full_until) op.template compute<U, false>(st, A, pos, stride, end);
+        else op.template compute<U, true>(st, A, pos, stride, end);
+        if (t + 1 < trips) {
+            if (t + 2 < trips) {
+#pragma unroll
+                for (int u = 0; u < U; ++u) op.load(A[u], ra[u], min(pos + 2 * step + u * stride, last));
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) rb[u] = tg_ldg_i32(idx + min(pos + 3 * step + u * stride, last));
+            if (pos + step < full_until) op.template compute<U, false>(st, B, pos + step, stride, end);
+            else op.template compute<U, true>(st, B, pos + step, stride, end);
+        }
+        pos += 2 * step;
+    }
+}
+
+// Warp tier: one warp per item {row, begin, end, slot}.
+template <class Op, int U, int MIN_CTAS>
+__global__ void __launch_bounds__(TG_CTA_THREADS, MIN_CTAS) tg_warp_kernel(typename Op::Params p, const int4* __restrict__ items,
+                                                                           const int32_t* __restrict__ indptr, int n_items) {
+    using Tr = typename Op::Tr;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int g = lane / Tr::LPR;
+    const int idx = blockIdx.x * TG_CTA_WARPS + warp;
+    if (idx >= n_items) return;
+    const int4 it = items[idx];
+    Op op(p, lane % Tr::LPR);
+    float st[Op::NS1];
+    op.init_row(it.x);
+    op.init_state(st);
+    const int n = it.z - it.y;
+    const int trips = (n + Tr::G * U - 1) / (Tr::G * U);
+    // a trip is full for every group when its last position (group G-1, edge U-1) is inside the chunk
+    const int full_until = it.y + g + ((n / (Tr::G * U)) * (Tr::G * U));
+    tg_run_edges_pipe<U>(op, st, it.y + g, it.z, Tr::G, trips, full_until);
+    tg_warp_merge(op, st);
+    if (lane < Tr::LPR) {
+        if (it.w < 0) op.write_final(it.x, st, true);
+        else op.write_partial(it.w, st, it.y == indptr[it.x]);
+    }
+}
+
+// Group tier: one group per record {row, begin, end, 0}.
+template <class Op, int U, int MIN_CTAS, bool PIPE>
+__global__ void __launch_bounds__(TG_CTA_THREADS, MIN_CTAS) tg_group_kernel(typename Op::Params p, const int4* __restrict__ rows,
+                                                                            int n_rows) {
+    using Tr = typename Op::Tr;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int g = lane / Tr::LPR;
+    const int idx = (blockIdx.x * TG_CTA_WARPS + warp) * Tr::G + g;
+    if (idx - g >= n_rows) return;  // the whole warp is idle
+    const bool active = idx < n_rows;
+    int4 it = make_int4(0, 0, 0, 0);  // an idle group re-reads row 0 and writes nothing
+    if (active) it = rows[idx];
+    Op op(p, lane % Tr::LPR);
+    float st[Op::NS1];
+    op.init_row(it.x);
+    op.init_state(st);
+    const int trips = __reduce_max_sync(0xffffffffu, (it.z - it.y + U - 1) / U);
+    if constexpr (PIPE) tg_run_edges_pipe<U>(op, st, it.y, it.z, 1, trips, it.y);
+    else tg_run_edges_plain<U>(op, st, it.y, it.z, 1, trips);
+    if (active) op.write_final(it.x, st, true);
+}
+
+// Hub merge.  A hub with <= TG_HUB_DIRECT chunks is folded by one CTA: every (warp, group) takes a strided
+// subset of the hub's partial slots.  Larger hubs (a hot source row can have thousands of chunks) are folded
+// in two levels: TG_HUB_SPLIT CTAs per hub write second-level partials (slots n_slots + hub*TG_HUB_SPLIT + j),
+// then one CTA per hub folds those.  level 0: single pass for every hub (no hub above TG_HUB_DIRECT);
+// level 1: blockIdx.y = j of the split pass (small hubs are finished here by j == 0); level 2: second pass.
+constexpr int TG_HUB_DIRECT = 32;
+constexpr int TG_HUB_SPLIT = 16;
+
 template <class Op>
-__global__ void __launch_bounds__(TG_CTA_THREADS) tg_hub_kernel(typename Op::Params p, SideDev sd) {
+__global__ void __launch_bounds__(TG_CTA_THREADS) tg_hub_kernel(typename Op::Params p, const int4* __restrict__ hubs, int n_slots,
+                                                                int level) {
     using Tr = typename Op::Tr;
     static_assert(Op::NS > 0, "an operator without state has no partials");
     __shared__ float sm[TG_CTA_WARPS * Tr::LPR * Op::NS];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int g = lane / Tr::LPR;
+    const int4 hub = hubs[blockIdx.x];  // row, first_slot, n_chunks
+    const bool big = hub.z > TG_HUB_DIRECT;
+    int first = hub.y, n = hub.z, start = 0, stride = 1, out_slot = -1;
+    if (level == 1) {
+        if (big) { start = blockIdx.y; stride = TG_HUB_SPLIT; out_slot = n_slots + blockIdx.x * TG_HUB_SPLIT + blockIdx.y; }
+        else if (blockIdx.y != 0) return;
+    } else if (level == 2) {
+        if (!big) return;
+        first = n_slots + blockIdx.x * TG_HUB_SPLIT; n = TG_HUB_SPLIT;
+    }
     Op op(p, lane % Tr::LPR);
-    const int4 hub = sd.hubs[blockIdx.x];  // row, first_slot, n_chunks
     float st[Op::NS];
     op.init_state(st);
-    for (int c = warp * Tr::G + g; c < hub.z; c += TG_CTA_WARPS * Tr::G) {
+    for (int c = start + (warp * Tr::G + g) * stride; c < n; c += TG_CTA_WARPS * Tr::G * stride) {
         float other[Op::NS];
-        op.load_partial(hub.y + c, other);
+        op.load_partial(first + c, other);
         op.merge(st, other);
     }
     tg_warp_merge(op, st);
     tg_cta_merge(op, st, sm, warp, lane);
-    if (warp == 0 && lane < Tr::LPR) op.write_final(hub.x, st, false);
+    if (warp == 0 && lane < Tr::LPR) {
+        if (out_slot < 0) op.write_final(hub.x, st, false);
+        else op.write_partial(out_slot, st, false);
+    }
 }
 
 // generic partial store / load: [slot][NS][LPR] fp32, lane-minor
@@ -153,25 +224,47 @@ __device__ __forceinline__ void tg_partial_load(const float* part, int slot, int
     for (int i = 0; i < NS; ++i) st[i] = p[i * Tr::LPR];
 }
 
-// Launch helper: tier kernel + (if the side has hubs) the hub merge.
-template <class Op>
+// Launch policy of one operator: edges per trip (U) and minimum resident CTAs per SM for the pipelined
+// (warp tier, big group classes) and the plain (small group classes) variants.
+template <int U_PIPE_, int CTAS_PIPE_, int U_PLAIN_, int CTAS_PLAIN_>
+struct TierPolicy {
+    static constexpr int U_PIPE = U_PIPE_, CTAS_PIPE = CTAS_PIPE_, U_PLAIN = U_PLAIN_, CTAS_PLAIN = CTAS_PLAIN_;
+};
+
+// Launch helper: all tiers of one side.
+template <class Op, class Pol>
 static tg_status_t tg_launch_tiers(const typename Op::Params& p, const tg_side& s, cudaStream_t stream, const char* name) {
     using Tr = typename Op::Tr;
     if (s.n_rows == 0) return TG_OK;
-    SideDev sd = tg_side_dev(s);
-    const int nb_warp = (s.n_warp + TG_CTA_WARPS - 1) / TG_CTA_WARPS;
-    const int nb_small = (s.n_small + TG_CTA_WARPS * Tr::G - 1) / (TG_CTA_WARPS * Tr::G);
-    const long long grid = (long long)s.n_items + nb_warp + nb_small;
-    if (grid > 0x7fffffffLL) TG_FAIL(TG_ERR_INTERNAL, "%s: grid too large", name);
-    if (grid > 0) {
-        tg_tier_kernel<Op><<<(unsigned)grid, TG_CTA_THREADS, 0, stream>>>(p, sd, nb_warp);
+    if (s.n_items > 0) {
+        const unsigned grid = (unsigned)((s.n_items + TG_CTA_WARPS - 1) / TG_CTA_WARPS);
+        tg_warp_kernel<Op, Pol::U_PIPE, Pol::CTAS_PIPE><<<grid, TG_CTA_THREADS, 0, stream>>>(p, s.items, s.indptr, s.n_items);
         TG_LAUNCH_CHECK(name);
     }
     if constexpr (Op::NS > 0) {
         if (s.n_hubs > 0) {
-            tg_hub_kernel<Op><<<(unsigned)s.n_hubs, TG_CTA_THREADS, 0, stream>>>(p, sd);
-            TG_LAUNCH_CHECK(name);
+            if (s.max_deg <= TG_HUB_DIRECT * TG_CHUNK) {
+                tg_hub_kernel<Op><<<(unsigned)s.n_hubs, TG_CTA_THREADS, 0, stream>>>(p, s.hubs, s.n_slots, 0);
+                TG_LAUNCH_CHECK(name);
+            } else {
+                tg_hub_kernel<Op><<<dim3((unsigned)s.n_hubs, TG_HUB_SPLIT), TG_CTA_THREADS, 0, stream>>>(p, s.hubs, s.n_slots, 1);
+                TG_LAUNCH_CHECK(name);
+                tg_hub_kernel<Op><<<(unsigned)s.n_hubs, TG_CTA_THREADS, 0, stream>>>(p, s.hubs, s.n_slots, 2);
+                TG_LAUNCH_CHECK(name);
+            }
         }
+    }
+    constexpr int rows_per_cta = TG_CTA_WARPS * Tr::G;
+    const int n_big = s.n_group_big(), n_small = s.n_group_small();
+    if (n_big > 0) {
+        const unsigned grid = (unsigned)((n_big + rows_per_cta - 1) / rows_per_cta);
+        tg_group_kernel<Op, Pol::U_PIPE, Pol::CTAS_PIPE, true><<<grid, TG_CTA_THREADS, 0, stream>>>(p, s.rows, n_big);
+        TG_LAUNCH_CHECK(name);
+    }
+    if (n_small > 0) {
+        const unsigned grid = (unsigned)((n_small + rows_per_cta - 1) / rows_per_cta);
+        tg_group_kernel<Op, Pol::U_PLAIN, Pol::CTAS_PLAIN, false><<<grid, TG_CTA_THREADS, 0, stream>>>(p, s.rows + n_big, n_small);
+        TG_LAUNCH_CHECK(name);
     }
     return TG_OK;
 }

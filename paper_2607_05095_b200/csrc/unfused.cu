@@ -6,7 +6,7 @@
 //                                          are not used);  dw[e,h] = <dY[v(e)], X[r(e)]> = SDDMM(dY, X).
 #include "dispatch.cuh"
 
-constexpr int TG_UNF_UNR = 2;
+using UnfPolicy = TierPolicy<2, 2, 2, 3>;
 
 struct SddmmArgs {
     const tg_block* b;
@@ -18,12 +18,12 @@ struct SddmmArgs {
 template <class Tr>
 struct SddmmFn {
     static tg_status_t run(const SddmmArgs& a) {
-        using Op = SddmmOp<Tr, TG_UNF_UNR>;
+        using Op = SddmmOp<Tr>;
         using T = typename Tr::T;
         typename Op::Params p;
         p.A = static_cast<const T*>(a.A); p.B = static_cast<const T*>(a.B);
         p.idx = a.b->kv_row; p.s = a.s; p.scale = a.scale;
-        return tg_launch_tiers<Op>(p, a.b->dst, a.stream, "tg_sddmm");
+        return tg_launch_tiers<Op, UnfPolicy>(p, a.b->dst, a.stream, "tg_sddmm");
     }
 };
 
@@ -39,12 +39,12 @@ struct AggArgs {
 template <class Tr>
 struct AggFn {
     static tg_status_t run(const AggArgs& a) {
-        using Op = AggOp<Tr, TG_UNF_UNR>;
+        using Op = AggOp<Tr>;
         using T = typename Tr::T;
         typename Op::Params p;
         p.X = static_cast<const T*>(a.X); p.idx = a.idx; p.widx = a.widx; p.w = a.w;
         p.Y = static_cast<T*>(a.Y); p.part = a.part;
-        return tg_launch_tiers<Op>(p, *a.side, a.stream, "tg_aggregate");
+        return tg_launch_tiers<Op, UnfPolicy>(p, *a.side, a.stream, "tg_aggregate");
     }
 };
 
@@ -67,7 +67,7 @@ extern "C" tg_status_t tg_aggregate_fwd(const tg_block_t* b, int H, int D, tg_dt
     if (b->E > 0) TG_CHECK_ROWS(X);
     tg_geom g;
     TG_TRY(tg_get_geom(H, D, dtype, &g));
-    const size_t need = (size_t)b->dst.n_slots * g.NE * g.LPR * sizeof(float);
+    const size_t need = tg_part_slots(b->dst) * g.NE * g.LPR * sizeof(float);
     if (need > 0 && (!ws || ws_bytes < need)) TG_FAIL(TG_ERR_WORKSPACE, "aggregate fwd needs %zu workspace bytes", need);
     AggArgs a{&b->dst, X, b->kv_row, nullptr, w, Y, static_cast<float*>(ws), static_cast<cudaStream_t>(stream)};
     return tg_dispatch<AggFn>(H, D, dtype, a);
@@ -82,7 +82,7 @@ extern "C" tg_status_t tg_aggregate_bwd(const tg_block_t* b, int H, int D, tg_dt
     if (dw) TG_CHECK_ROWS(X);
     tg_geom g;
     TG_TRY(tg_get_geom(H, D, dtype, &g));
-    const size_t need = (size_t)b->src.n_slots * g.NE * g.LPR * sizeof(float);
+    const size_t need = tg_part_slots(b->src) * g.NE * g.LPR * sizeof(float);
     if (need > 0 && (!ws || ws_bytes < need)) TG_FAIL(TG_ERR_WORKSPACE, "aggregate bwd needs %zu workspace bytes", need);
     AggArgs a{&b->src, dY, b->t_dst, b->t_edge, w, dX, static_cast<float*>(ws), static_cast<cudaStream_t>(stream)};
     TG_TRY(tg_dispatch<AggFn>(H, D, dtype, a));
