@@ -22,6 +22,8 @@ LIB = os.path.join(HERE, "libfasttg.so")
 SOURCES = ["api.cu", "block.cu", "fused_fwd.cu", "fused_bwd.cu", "unfused.cu", "softmax.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--use_fast_math",
               "-Xcompiler", "-fPIC,-fvisibility=hidden", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
+# tuning knobs (e.g. TG_NVCC_EXTRA="-DTG_FWD_POLICY=1,3,1,4"); part of the build stamp
+NVCC_FLAGS += os.environ.get("TG_NVCC_EXTRA", "").split()
 
 
 def _nvcc() -> str:

@@ -129,6 +129,11 @@ __device__ __forceinline__ int tg_ldg_i32(const int32_t* p) {
     asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(r) : "l"(p));
     return r;
 }
+// load whose value is never used: brings the sector into L1 ahead of time (a CCTL prefetch serialises here)
+__device__ __forceinline__ void tg_touch_i32(const int32_t* p) {
+    int r;
+    asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(r) : "l"(p));
+}
 __device__ __forceinline__ float tg_ldg_f32(const float* p) {
     float r;
     asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(r) : "l"(p));

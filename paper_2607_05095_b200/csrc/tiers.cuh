@@ -77,8 +77,11 @@ __device__ __forceinline__ void tg_run_edges_plain(Op& op, float (&st)[Op::NS1],
 }
 
 // Software-pipelined edge loop with two register buffers: while trip t is computed the rows of trip t+1
-// are in flight and the row indices of trip t+2 are being fetched, so a warp exposes the gather latency
-// once per loop, not once per trip.  Positions past `end` are clamped for the loads (a valid row is fetched
+// are in flight, so a warp exposes the gather latency once per loop, not once per trip.  The row indices
+// are requested a whole iteration (two trips) before the row loads that use them: the per-edge index
+// stream enters a new 32-byte sector every few trips, each first touch is an L2/DRAM round trip, and a
+// single trip of lead does not cover it (measured: 25 % of the warp tier's stall samples sat on the
+// index -> address dependency).  Positions past `end` are clamped for the loads (a valid row is fetched
 // again) and masked in compute().  `full_until`: trips whose first position is below it need no mask
 // (warp-uniform; pass i0 to mask everything).
 template <int U, class Op>
@@ -88,34 +91,38 @@ __device__ __forceinline__ void tg_run_edges_pipe(Op& op, float (&st)[Op::NS1], 
     const int32_t* __restrict__ idx = op.idx_ptr();
     const int last = max(end - 1, 0);
     typename Op::Buf A[U], B[U];
-    int ra[U], rb[U];
+    int ia[U], ib[U], na[U], nb[U];   // indices of trips t+2, t+1 (used this iteration) and t+4, t+3 (next one)
     const int step = U * stride;
     int pos = i0;  // first position of the trip being computed
 #pragma unroll
-    for (int u = 0; u < U; ++u) ra[u] = tg_ldg_i32(idx + min(pos + u * stride, last));
+    for (int u = 0; u < U; ++u) na[u] = tg_ldg_i32(idx + min(pos + u * stride, last));
 #pragma unroll
-    for (int u = 0; u < U; ++u) op.load(A[u], ra[u], min(pos + u * stride, last));
+    for (int u = 0; u < U; ++u) ib[u] = tg_ldg_i32(idx + min(pos + step + u * stride, last));
 #pragma unroll
-    for (int u = 0; u < U; ++u) rb[u] = tg_ldg_i32(idx + min(pos + step + u * stride, last));
+    for (int u = 0; u < U; ++u) ia[u] = tg_ldg_i32(idx + min(pos + 2 * step + u * stride, last));
+#pragma unroll
+    for (int u = 0; u < U; ++u) op.load(A[u], na[u], min(pos + u * stride, last));
     for (int t = 0; t < trips; t += 2) {
+#pragma unroll
+        for (int u = 0; u < U; ++u) nb[u] = tg_ldg_i32(idx + min(pos + 3 * step + u * stride, last));
+#pragma unroll
+        for (int u = 0; u < U; ++u) na[u] = tg_ldg_i32(idx + min(pos + 4 * step + u * stride, last));
         if (t + 1 < trips) {
 #pragma unroll
-            for (int u = 0; u < U; ++u) op.load(B[u], rb[u], min(pos + step + u * stride, last));
+            for (int u = 0; u < U; ++u) op.load(B[u], ib[u], min(pos + step + u * stride, last));
         }
-#pragma unroll
-        for (int u = 0; u < U; ++u) ra[u] = tg_ldg_i32(idx + min(pos + 2 * step + u * stride, last));
         if (pos < full_until) op.template compute<U, false>(st, A, pos, stride, end);
         else op.template compute<U, true>(st, A, pos, stride, end);
         if (t + 1 < trips) {
             if (t + 2 < trips) {
 #pragma unroll
-                for (int u = 0; u < U; ++u) op.load(A[u], ra[u], min(pos + 2 * step + u * stride, last));
+                for (int u = 0; u < U; ++u) op.load(A[u], ia[u], min(pos + 2 * step + u * stride, last));
             }
-#pragma unroll
-            for (int u = 0; u < U; ++u) rb[u] = tg_ldg_i32(idx + min(pos + 3 * step + u * stride, last));
             if (pos + step < full_until) op.template compute<U, false>(st, B, pos + step, stride, end);
             else op.template compute<U, true>(st, B, pos + step, stride, end);
         }
+#pragma unroll
+        for (int u = 0; u < U; ++u) { ia[u] = na[u]; ib[u] = nb[u]; }
         pos += 2 * step;
     }
 }
