@@ -127,15 +127,15 @@ __device__ __forceinline__ float slot_pick(const float (&x)[Tr::NHL], const Lane
 template <class Tr, int k>
 __device__ __forceinline__ float slot_dot(const RowReg<Tr>& a, const RowReg<Tr>& b) {
     if constexpr (Tr::BF16) {
-        float acc = 0.f;
+        float acc0 = 0.f, acc1 = 0.f;   // two chains: the FHFMA result latency is not exposed back to back
 #pragma unroll
         for (int i = Tr::WV * k; i < Tr::WV * (k + 1); ++i) {
             asm("{\n\t.reg .b16 al, ah, bl, bh;\n\t"
-                "mov.b32 {al, ah}, %1;\n\tmov.b32 {bl, bh}, %2;\n\t"
-                "fma.rn.f32.bf16 %0, al, bl, %0;\n\tfma.rn.f32.bf16 %0, ah, bh, %0;\n\t}"
-                : "+f"(acc) : "r"(a.w[i]), "r"(b.w[i]));
+                "mov.b32 {al, ah}, %2;\n\tmov.b32 {bl, bh}, %3;\n\t"
+                "fma.rn.f32.bf16 %0, al, bl, %0;\n\tfma.rn.f32.bf16 %1, ah, bh, %1;\n\t}"
+                : "+f"(acc0), "+f"(acc1) : "r"(a.w[i]), "r"(b.w[i]));
         }
-        return acc;
+        return acc0 + acc1;
     } else {
         static_assert(Tr::BF16 || Tr::WV % 2 == 0, "fp32 vectors hold an even number of elements");
         float acc0 = 0.f, acc1 = 0.f;
