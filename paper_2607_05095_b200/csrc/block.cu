@@ -24,13 +24,14 @@ constexpr int TG_SK = TG_NCLS + 3;
 
 struct SchedIn {
     const int32_t* indptr;
+    int chunk;
     __device__ __forceinline__ IVec<TG_SK> operator()(int64_t i) const {
         const int deg = indptr[i + 1] - indptr[i];
         IVec<TG_SK> x = ivec_zero<TG_SK>();
         if (deg <= TG_GROUP_MAX) {
             x.v[tg_degree_class(deg)] = 1;
         } else {
-            const int chunks = (deg + TG_CHUNK - 1) / TG_CHUNK;
+            const int chunks = (deg + chunk - 1) / chunk;
             x.v[TG_NCLS] = chunks;
             x.v[TG_NCLS + 1] = chunks > 1 ? chunks : 0;
             x.v[TG_NCLS + 2] = chunks > 1;
@@ -65,8 +66,9 @@ struct SchedOut {
     }
 };
 
-static inline int64_t side_items_bound(int64_t n_edges) { return n_edges / TG_GROUP_MAX + 2; }
-static inline int64_t side_hubs_bound(int64_t n_edges) { return n_edges / TG_CHUNK + 1; }
+// a warp-tier row (deg > TG_GROUP_MAX) has ceil(deg / chunk) <= deg / TG_CHUNK_MIN + 1 <= 2 * deg / TG_GROUP_MAX items
+static inline int64_t side_items_bound(int64_t n_edges) { return 2 * (n_edges / TG_GROUP_MAX) + 2; }
+static inline int64_t side_hubs_bound(int64_t n_edges) { return n_edges / TG_CHUNK_MIN + 1; }
 
 size_t tg_side_bytes(int64_t n_rows_bound, int64_t n_edges) {
     return tg_align_up((size_t)(n_rows_bound + 1) * sizeof(int4)) + tg_align_up((size_t)side_items_bound(n_edges) * sizeof(int4)) +
@@ -86,7 +88,11 @@ tg_status_t tg_side_build(tg_side* s, int64_t n_rows, int64_t n_edges, const int
     int* totals = static_cast<int*>(c.take(256));  // IVec<TG_SK> + max_deg at [TG_SK]
     if (!c.ok()) TG_FAIL(TG_ERR_WORKSPACE, "schedule workspace too small: need %zu, have %zu", c.off, ws_bytes);
     TG_CUDA(cudaMemsetAsync(totals, 0, 256, stream));
-    SchedIn in{indptr};
+    // about 4 warp items per resident warp slot (148 SMs x 16 warps) when the side is small, TG_CHUNK_MAX beyond
+    int chunk = TG_CHUNK_MIN;
+    while (chunk < TG_CHUNK_MAX && n_edges / chunk > 148 * 16 * 4) chunk *= 2;
+    s->chunk = chunk;
+    SchedIn in{indptr, chunk};
     SchedOut out{indptr, s->rows, s->items, s->hubs, totals + TG_SK};
     TG_TRY((tg_scan<TG_SK>(n_rows, in, out, scan_tmp, reinterpret_cast<IVec<TG_SK>*>(totals), stream)));
     int h[TG_SK + 1];

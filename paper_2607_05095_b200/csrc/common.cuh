@@ -53,14 +53,16 @@ void tg_count_launch();
 //   group tier: deg <= TG_GROUP_MAX    one sub-warp group per row (the K <= 10-20 common case); rows are
 //                                      bucketed into TG_NCLS power-of-two degree classes so that the
 //                                      groups of a warp run the same number of trips
-//   warp tier : larger                 one warp per chunk of <= TG_CHUNK edges; a row with more than one
+//   warp tier : larger                 one warp per chunk of <= `chunk` edges (TG_CHUNK_MIN..TG_CHUNK_MAX, picked per
+//                                      side so that a small block still spreads over the SMs: a lone warp walks
+//                                      its chunk as one latency chain); a row with more than one
 //                                      chunk ("hub") writes fp32 partials, merged by a second launch
 // Every schedule record carries {row, begin, end}: one load instead of the order -> indptr chain.
 // ---------------------------------------------------------------------------------------------
 constexpr int TG_NCLS = 6;          // degree classes <=2, 3-4, 5-8, 9-16, 17-32, 33-64
 constexpr int TG_NCLS_SMALL = 3;    // classes 0..2 (deg <= 8) run in the high-occupancy kernel variant
 constexpr int TG_GROUP_MAX = 64;
-constexpr int TG_CHUNK = 512;
+constexpr int TG_CHUNK_MIN = 64, TG_CHUNK_MAX = 512;
 constexpr int TG_CTA_THREADS = 256;
 constexpr int TG_CTA_WARPS = TG_CTA_THREADS / 32;
 
@@ -77,6 +79,7 @@ struct tg_side {
     int32_t n_cls[TG_NCLS] = {0, 0, 0, 0, 0, 0};
     int32_t n_group = 0, n_items = 0, n_hubs = 0, n_slots = 0;
     int32_t max_deg = 0;
+    int32_t chunk = TG_CHUNK_MAX;   // edges per warp item of this side
     // group-tier rows of the classes >= TG_NCLS_SMALL come first in `rows`
     int32_t n_group_big() const { int n = 0; for (int c = TG_NCLS_SMALL; c < TG_NCLS; ++c) n += n_cls[c]; return n; }
     int32_t n_group_small() const { return n_group - n_group_big(); }

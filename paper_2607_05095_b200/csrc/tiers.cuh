@@ -1,7 +1,7 @@
 // tiers.cuh -- the degree-tiered driver shared by every row-gather operator.
 //
 // A CSR side is covered by up to four launches (largest work first):
-//   tg_warp_kernel   warp tier : one warp per chunk (<= TG_CHUNK edges) of a large row; its G groups stride
+//   tg_warp_kernel   warp tier : one warp per chunk (<= tg_side::chunk edges) of a large row; its G groups stride
 //                                over the chunk's edges, states are merged by shuffles; a hub (row with
 //                                several chunks) writes an fp32 partial per chunk
 //   tg_hub_kernel    folds each hub's partials (two levels when a hub has more than TG_HUB_DIRECT chunks)
@@ -250,7 +250,7 @@ static tg_status_t tg_launch_tiers(const typename Op::Params& p, const tg_side& 
     }
     if constexpr (Op::NS > 0) {
         if (s.n_hubs > 0) {
-            if (s.max_deg <= TG_HUB_DIRECT * TG_CHUNK) {
+            if (s.max_deg <= TG_HUB_DIRECT * s.chunk) {
                 tg_hub_kernel<Op><<<(unsigned)s.n_hubs, TG_CTA_THREADS, 0, stream>>>(p, s.hubs, s.n_slots, 0);
                 TG_LAUNCH_CHECK(name);
             } else {

@@ -76,7 +76,10 @@ def test_block_build_bit_exact(B, oracle_mod, w, dedup):
     assert info["R"] == w.R and info["E"] == w.E and info["U"] == ob.U
     deg = np.diff(ob.indptr)
     assert info["dst_group_small"] == int((deg <= 8).sum()) and info["dst_group_big"] == int(((deg > 8) & (deg <= 64)).sum())
-    assert info["dst_warp_items"] == int(np.ceil(deg[deg > 64] / 512).sum())
+    chunk = 64
+    while chunk < 512 and w.E // chunk > 148 * 16 * 4:
+        chunk *= 2
+    assert info["dst_warp_items"] == int(np.ceil(deg[deg > 64] / chunk).sum())
 
 
 def test_block_build_negative_ids_and_empty(B, oracle_mod):
@@ -124,7 +127,7 @@ def test_fused_all_tiers_with_hubs(B, oracle_mod, H, D, dtype):
     ob = _oblock(oracle_mod, w)
     gb = gpu_block(B, w)
     info = gb.info()
-    assert info["dst_slots"] >= 4 and info["src_slots"] >= 2 and info["dst_warp_items"] > info["dst_slots"]
+    assert info["dst_slots"] >= 4 and info["src_slots"] >= 2 and info["dst_warp_items"] >= info["dst_slots"]
     feats = w.features(ob.U)
     scale = float(math.sqrt(D))                                              # logits ~ N(0,1): softmax far from uniform
     got = run_fused(B, gb, w, feats, scale)
