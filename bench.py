@@ -42,8 +42,13 @@ def measured_hbm_gbs():
     return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)"
 
 
-def make_workloads(cfg: int, seed: int):
+def make_workloads(cfg: int, seed: int, src_nodes: int = 0):
     from paper_2607_05095_b200 import workloads as W
+    if src_nodes > 0:   # diagnostic: config 4's degree structure over `src_nodes` source nodes (16: every gather hits L1)
+        assert cfg == 4, "--src-nodes is a config-4 diagnostic"
+        w = W.config4(seed, n_src_nodes=src_nodes)
+        w.name += f"_src{src_nodes}"
+        return [w]
     if cfg == 1:
         return [W.config1(seed)]
     if cfg == 2:
@@ -182,7 +187,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     B.lib()
 
-    ws = make_workloads(args.config, args.seed + rank)          # each rank: its own independent mini-batch
+    ws = make_workloads(args.config, args.seed + rank, args.src_nodes)          # each rank: its own independent mini-batch
     TDT = {"f32": torch.float32, "bf16": torch.bfloat16}
     blocks = []
     for w in ws:
@@ -272,13 +277,14 @@ def run_ours(args):
     kb = kernel_bytes(w.R, w.E, b["blk"].U, w.H, w.D, eb, w.dedup_mode)
     dom = max(per_block[bi_dom], key=per_block[bi_dom].get)
     achieved = kb[dom] / (per_block[bi_dom][dom] * 1e-3) / 1e9
+    # DRAM bytes of the dominant call from the committed ncu capture (profiles/traffic.csv), per call like `achieved`
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    tp = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(tp):
-        try:
-            traffic = json.load(open(tp)).get(f"config{args.config}", {}).get(dom)
-        except Exception:
-            traffic = None
+        for ln in open(tp).read().splitlines()[1:]:
+            f = ln.split(",")
+            if len(f) >= 3 and f[0] == str(args.config) and f[1] == dom:
+                traffic = int(f[2])
     roofline = {"bound": "hbm", "kernel": {"fwd": "tg_attn_fused_fwd", "bwd_dst": "tg_attn_fused_bwd_dst", "bwd_src": "tg_attn_fused_bwd_src"}[dom]
                 + f" = tg_warp_kernel + tg_hub_kernel + 2 x tg_group_kernel <{ {'fwd': 'FwdOp', 'bwd_dst': 'Bwd1Op', 'bwd_src': 'Bwd2Op'}[dom] }>", "achieved": achieved,
                 "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
@@ -400,6 +406,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-edges", type=int, default=2_000_000)
     ap.add_argument("--ref-edges", type=int, default=1_000_000)
+    ap.add_argument("--src-nodes", type=int, default=0, help="diagnostic (config 4): number of source nodes; not the headline workload")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-unfused", action="store_true")
     args = ap.parse_args()
