@@ -172,6 +172,20 @@ def run_reference(args):
 # ---------------------------------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------------------------------
+def reduce_over_ranks(total_ms: float, edges_local: int, world: int, device: str):
+    """Replicas only: every rank times its own independent mini-batch; the job's time is the MAX over
+    ranks and its work the SUM of the ranks' edges.  No data-path collective."""
+    if world <= 1:
+        return total_ms, edges_local
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([total_ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e = torch.tensor([edges_local], device=device, dtype=torch.int64)
+    dist.all_reduce(e)
+    return float(t.item()), int(e.item())
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -237,17 +251,9 @@ def run_ours(args):
     barrier()
     total_ms = t_start.elapsed_time(t_end)
     clocks = sampler.stop() if rank == 0 else None
-    if world > 1:
-        t = torch.tensor([total_ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-    ms_per_step = total_ms / args.steps
     E_local = sum(b["w"].E for b in blocks)
-    E_all = E_local
-    if world > 1:
-        t = torch.tensor([E_local], device="cuda", dtype=torch.int64)
-        dist.all_reduce(t)
-        E_all = int(t.item())
+    total_ms, E_all = reduce_over_ranks(total_ms, E_local, world, "cuda")
+    ms_per_step = total_ms / args.steps
     value = E_all / (ms_per_step * 1e-3)
 
     # per-kernel durations (this rank), averaged over the timed steps

@@ -1,0 +1,98 @@
+"""`-m "not gpu"`: the C-ABI library loads and exports every symbol include/fasttg.h declares, the host-only
+entry points behave as the header says (no compute call is made without a GPU), and the N > 1 host logic of
+bench.py (replicas only: max time, summed edges; reference arm on rank 0 alone) runs under gloo with world size 2."""
+import ctypes as C
+import json
+import os
+import re
+import subprocess
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def L():
+    from paper_2607_05095_b200 import build, binding
+    build.build()
+    return binding.lib()
+
+
+def _declared():
+    text = open(os.path.join(ROOT, "include", "fasttg.h")).read()
+    return sorted(set(re.findall(r"TG_API\s+[\w\s\*]+?\b(tg_\w+)\s*\(", text)))
+
+
+def test_every_declared_symbol_is_exported(L):
+    from paper_2607_05095_b200 import binding
+    names = _declared()
+    assert len(names) >= 20 and "tg_attn_fused_fwd" in names and "tg_block_build" in names and "tg_launch_count" in names
+    for n in names:
+        assert hasattr(L, n), f"{n} declared in include/fasttg.h but not exported by libfasttg.so"
+    assert sorted(binding.EXPORTS) == names, "binding.EXPORTS and include/fasttg.h disagree"
+
+
+def test_host_only_entry_points(L):
+    assert L.tg_version() >= 100
+    assert L.tg_status_string(0) == b"TG_OK" and L.tg_status_string(5) == b"TG_ERR_CUDA"
+    for H, D in ((2, 50), (4, 32), (8, 16), (2, 64)):                    # the shapes BASELINE.json's configs need
+        assert L.tg_supported(H, D, 0) == 1 and L.tg_supported(H, D, 1) == 1
+    assert L.tg_supported(3, 7, 0) == 0 and L.tg_supported(8, 16, 9) == 0
+    n = C.c_size_t(0)
+    st = L.tg_block_workspace_bytes(C.c_int64(1000), C.c_int64(10000), 1, C.byref(n))
+    assert st in (0, 5)          # the size query asks cub for its temp size: TG_ERR_CUDA on a box without a device
+    if st == 0:
+        small = n.value
+        assert small > 10000 * 24
+        assert L.tg_block_workspace_bytes(C.c_int64(1000), C.c_int64(20000), 1, C.byref(n)) == 0 and n.value > small
+    else:
+        assert L.tg_last_error() != b""
+    assert L.tg_block_workspace_bytes(C.c_int64(-1), C.c_int64(10), 1, C.byref(n)) == 1      # TG_ERR_INVALID_ARG
+    assert b"out of range" in L.tg_last_error()
+    assert L.tg_block_workspace_bytes(C.c_int64(10), C.c_int64(10), 1, None) == 1
+    assert L.tg_sched_workspace_bytes(C.c_int64(10), C.c_int64(100), C.c_int64(50), C.byref(n)) == 0 and n.value > 0
+    before = L.tg_launch_count()
+    # argument validation happens before any launch: null block -> error, no launch counted
+    assert L.tg_attn_fused_fwd(None, 8, 16, 1, None, None, None, C.c_float(1.0), None, None, None, C.c_size_t(0), None) == 1
+    assert L.tg_launch_count() == before
+
+
+_WORKER = r"""
+import os, sys
+sys.path.insert(0, os.environ["TG_ROOT"])
+import torch.distributed as dist
+import bench
+dist.init_process_group("gloo", rank=int(os.environ["RANK"]), world_size=int(os.environ["WORLD_SIZE"]))
+r = dist.get_rank()
+ms, edges = bench.reduce_over_ranks(10.0 + 5.0 * r, 1000 * (r + 1), dist.get_world_size(), "cpu")
+assert ms == 15.0 and edges == 3000, (ms, edges)
+ws0 = bench.make_workloads(1, 0 + r)            # each rank: its own mini-batch (seed + rank)
+print("rank", r, "ok", ws0[0].E)
+dist.barrier(); dist.destroy_process_group()
+"""
+
+
+def test_replica_reduction_gloo_world2(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(_WORKER)
+    procs = []
+    for r in range(2):
+        env = dict(os.environ, RANK=str(r), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1", MASTER_PORT="29517", TG_ROOT=ROOT)
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True))
+    outs = [p.communicate(timeout=300)[0] for p in procs]
+    assert all(p.returncode == 0 for p in procs), outs
+    e = [int(o.strip().split()[-1]) for o in outs]
+    assert e[0] != e[1], "ranks must draw different mini-batches"
+
+
+def test_reference_arm_runs_on_rank0_only():
+    base = [sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "1", "--gpus", "2", "--steps", "1", "--warmup", "0"]
+    r1 = subprocess.run(base, env=dict(os.environ, RANK="1", WORLD_SIZE="2"), capture_output=True, text=True, timeout=300)
+    assert r1.returncode == 0 and r1.stdout.strip() == ""
+    r0 = subprocess.run(base, env=dict(os.environ, RANK="0", WORLD_SIZE="2"), capture_output=True, text=True, timeout=300)
+    assert r0.returncode == 0, r0.stderr
+    line = json.loads(r0.stdout.strip().splitlines()[-1])
+    assert line["impl"] == "reference" and line["cpu_baseline"]["kind"] == "oracle" and line["value"] > 0
+    assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["unit"] == "edges/s"
