@@ -4,12 +4,32 @@
 #include "dispatch.cuh"
 
 // launch policy {edges per trip, min CTAs per SM} for the pipelined and the plain kernel variants
-#ifndef TG_BWD1_POLICY
-#define TG_BWD1_POLICY 1, 2, 1, 3
+#ifndef TG_BWD1_U
+#define TG_BWD1_U 1
 #endif
-#ifndef TG_BWD2_POLICY
-#define TG_BWD2_POLICY 1, 2, 1, 3
+#ifndef TG_BWD1_CTAS
+#define TG_BWD1_CTAS 2
 #endif
+#ifndef TG_BWD1_UP
+#define TG_BWD1_UP 1
+#endif
+#ifndef TG_BWD1_CTASP
+#define TG_BWD1_CTASP 3
+#endif
+#define TG_BWD1_POLICY TG_BWD1_U, TG_BWD1_CTAS, TG_BWD1_UP, TG_BWD1_CTASP
+#ifndef TG_BWD2_U
+#define TG_BWD2_U 1
+#endif
+#ifndef TG_BWD2_CTAS
+#define TG_BWD2_CTAS 2
+#endif
+#ifndef TG_BWD2_UP
+#define TG_BWD2_UP 1
+#endif
+#ifndef TG_BWD2_CTASP
+#define TG_BWD2_CTASP 3
+#endif
+#define TG_BWD2_POLICY TG_BWD2_U, TG_BWD2_CTAS, TG_BWD2_UP, TG_BWD2_CTASP
 
 struct BwdArgs {
     const tg_block* b;

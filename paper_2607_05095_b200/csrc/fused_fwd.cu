@@ -3,9 +3,19 @@
 #include "dispatch.cuh"
 
 // launch policy {edges per trip, min CTAs per SM} for the pipelined and the plain kernel variants
-#ifndef TG_FWD_POLICY
-#define TG_FWD_POLICY 2, 2, 2, 3
+#ifndef TG_FWD_U
+#define TG_FWD_U 2
 #endif
+#ifndef TG_FWD_CTAS
+#define TG_FWD_CTAS 2
+#endif
+#ifndef TG_FWD_UP
+#define TG_FWD_UP 2
+#endif
+#ifndef TG_FWD_CTASP
+#define TG_FWD_CTASP 3
+#endif
+#define TG_FWD_POLICY TG_FWD_U, TG_FWD_CTAS, TG_FWD_UP, TG_FWD_CTASP
 
 struct FwdArgs {
     const tg_block* b;
