@@ -413,9 +413,16 @@ def main():
     ap.add_argument("--cpu-edges", type=int, default=2_000_000)
     ap.add_argument("--ref-edges", type=int, default=1_000_000)
     ap.add_argument("--src-nodes", type=int, default=0, help="diagnostic (config 4): number of source nodes; not the headline workload")
+    ap.add_argument("--probe-gather", action="store_true", help="diagnostic: print the measured L1 / L2 row-gather bandwidth and exit")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-unfused", action="store_true")
     args = ap.parse_args()
+    if args.probe_gather:
+        from paper_2607_05095_b200 import binding as B
+        rows = {"l1_64rows_16KB": 64, "l1_512rows_128KB": 512, "l2_65536rows_16MB": 65536, "dram_8Mrows_2GB": 8 << 20}
+        print(json.dumps({"probe": "256-byte row gathers, 8 lanes x 2 LDG.128 per row", "unit": "GB/s",
+                          **{k: round(B.probe_gather(v), 1) for k, v in rows.items()}}))
+        return
     if args.impl == "reference":
         run_reference(args)
     else:

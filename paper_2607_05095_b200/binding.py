@@ -20,7 +20,7 @@ TG_F32, TG_BF16 = 0, 1
 _DTYPES = {torch.float32: TG_F32, torch.bfloat16: TG_BF16}
 
 EXPORTS = [
-    "tg_status_string", "tg_last_error", "tg_version", "tg_supported", "tg_launch_count",
+    "tg_status_string", "tg_last_error", "tg_version", "tg_supported", "tg_launch_count", "tg_probe_gather",
     "tg_block_workspace_bytes", "tg_block_build", "tg_sched_workspace_bytes", "tg_block_from_csr",
     "tg_block_destroy", "tg_block_info",
     "tg_sddmm", "tg_edge_softmax_fwd", "tg_edge_softmax_bwd", "tg_aggregate_fwd", "tg_aggregate_bwd",
@@ -53,6 +53,16 @@ def lib() -> C.CDLL:
 def launch_count() -> int:
     """tg_launch_count: kernels launched by the library in this process so far."""
     return int(lib().tg_launch_count())
+
+
+def probe_gather(table_rows: int, gathers_per_group: int = 4096, iters: int = 5) -> float:
+    """tg_probe_gather: GB/s of 256-byte row gathers from a table of `table_rows` rows (small: all L1 hits)."""
+    table = torch.randint(0, 2 ** 31 - 1, (table_rows, 64), dtype=torch.int32, device="cuda")
+    sink = torch.zeros(1, dtype=torch.int32, device="cuda")
+    ms, nbytes = C.c_float(0), C.c_double(0)
+    _check(lib().tg_probe_gather(_ptr(table), C.c_int(table_rows), C.c_int(gathers_per_group), C.c_int(iters), _ptr(sink),
+                                 _stream(), C.byref(ms), C.byref(nbytes)), "tg_probe_gather")
+    return nbytes.value / (ms.value * 1e-3) / 1e9
 
 
 def _check(st: int, where: str):

@@ -36,3 +36,49 @@ extern "C" const char* tg_status_string(tg_status_t s) {
 extern "C" int tg_version(void) { return 100; }
 
 extern "C" int tg_supported(int H, int D, tg_dtype_t dtype) { return tg_shape_supported(H, D, dtype) ? 1 : 0; }
+
+// ---------------------------------------------------------------------------------------------
+// tg_probe_gather: measures the L1 gather roof that the row-gather kernels sit against.  Every group of
+// 8 lanes reads one 256-byte row (two LDG.128 per lane, one 128-byte line per group and instruction -- the
+// access shape of rowops.cuh) at a pseudo-random index of a table of `table_rows` rows and xors it into a
+// register; table_rows small => every access hits L1.  Returns the time of `iters` launches.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_probe_gather(const uint4* __restrict__ table, int table_rows, int gathers_per_group,
+                                                       uint32_t* sink) {
+    const int lane = threadIdx.x & 31, lig = lane & 7;
+    uint32_t h = (blockIdx.x * blockDim.x + threadIdx.x) >> 3;   // group id
+    uint4 acc = make_uint4(0, 0, 0, 0);
+#pragma unroll 4
+    for (int i = 0; i < gathers_per_group; ++i) {
+        h = h * 1664525u + 1013904223u;
+        const uint4* row = table + (size_t)((h >> 8) % (uint32_t)table_rows) * 16;   // 16 x 16 bytes per row
+        const uint4 a = tg_ldg128(row + lig), b = tg_ldg128(row + lig + 8);
+        acc.x ^= a.x ^ b.x; acc.y ^= a.y ^ b.y; acc.z ^= a.z ^ b.z; acc.w ^= a.w ^ b.w;
+    }
+    if ((acc.x ^ acc.y ^ acc.z ^ acc.w) == 0x12345678u) sink[0] = acc.x;   // keeps the loads alive
+}
+
+extern "C" tg_status_t tg_probe_gather(const void* table, int table_rows, int gathers_per_group, int iters, void* sink,
+                                       tg_stream_t stream_, float* ms, double* bytes) {
+    if (!table || !sink || !ms || !bytes || table_rows < 1 || gathers_per_group < 1 || iters < 1)
+        TG_FAIL(TG_ERR_INVALID_ARG, "tg_probe_gather: bad argument");
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    const int grid = 148 * 8;   // 8 CTAs of 256 threads per SM
+    cudaEvent_t e0, e1;
+    TG_CUDA(cudaEventCreate(&e0));
+    TG_CUDA(cudaEventCreate(&e1));
+    k_probe_gather<<<grid, 256, 0, stream>>>(static_cast<const uint4*>(table), table_rows, gathers_per_group, static_cast<uint32_t*>(sink));
+    TG_LAUNCH_CHECK("k_probe_gather");
+    TG_CUDA(cudaEventRecord(e0, stream));
+    for (int i = 0; i < iters; ++i) {
+        k_probe_gather<<<grid, 256, 0, stream>>>(static_cast<const uint4*>(table), table_rows, gathers_per_group, static_cast<uint32_t*>(sink));
+        TG_LAUNCH_CHECK("k_probe_gather");
+    }
+    TG_CUDA(cudaEventRecord(e1, stream));
+    TG_CUDA(cudaEventSynchronize(e1));
+    TG_CUDA(cudaEventElapsedTime(ms, e0, e1));
+    TG_CUDA(cudaEventDestroy(e0));
+    TG_CUDA(cudaEventDestroy(e1));
+    *bytes = (double)iters * grid * 32.0 /*groups per CTA*/ * gathers_per_group * 256.0;
+    return TG_OK;
+}
