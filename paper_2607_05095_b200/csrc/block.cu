@@ -21,12 +21,18 @@
 // ---------------------------------------------------------------------------------------------
 // scan vector: [0, TG_NCLS) group-tier class counts, then warp items per length class (TG_NICLS), partial slots, hubs.
 // Warp items are stored by length class, longest first -- class 0: chunks of multi-chunk rows (chunk/2 < len <= chunk),
-// then single-chunk rows by halving length -- so that the 8 warps of a CTA finish together (the CTA's registers are
+// then single-chunk rows in classes of a factor sqrt(2) in length -- so that the 8 warps of a CTA finish together (the CTA's registers are
 // held until its slowest warp ends: unsorted items left 30 % of the resident warp slots idle on config 4).
-constexpr int TG_NICLS = 4;
+constexpr int TG_NICLS = 7;
 constexpr int TG_SK = TG_NCLS + TG_NICLS + 2;
 __host__ __device__ constexpr int tg_item_class(int deg, int chunk) {
-    return deg > chunk ? 0 : (2 * deg > chunk ? 1 : (4 * deg > chunk ? 2 : 3));
+    if (deg > chunk) return 0;
+    int c = 1;   // single-chunk rows: one class per factor sqrt(2) of length (181/256 ~ 1/sqrt 2)
+    for (int t = chunk; c < TG_NICLS - 1; ++c) {
+        t = (c & 1) ? (chunk >> (c >> 1)) * 181 >> 8 : chunk >> (c >> 1);
+        if (deg > t) break;
+    }
+    return c;
 }
 
 struct SchedIn {
