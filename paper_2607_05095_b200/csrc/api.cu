@@ -20,6 +20,24 @@ static std::atomic<unsigned long long> g_launches{0};
 void tg_count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
 extern "C" unsigned long long tg_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
+tg_aux_streams* tg_get_aux_streams() {
+    static thread_local tg_aux_streams aux;
+    static thread_local int dev = -1;
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess) { tg_set_error("cudaGetDevice failed"); return nullptr; }
+    if (dev != cur) {   // first use on this thread / device
+        bool ok = true;
+        for (int i = 0; i < 2; ++i) {
+            ok = ok && cudaStreamCreateWithFlags(&aux.s[i], cudaStreamNonBlocking) == cudaSuccess;
+            ok = ok && cudaEventCreateWithFlags(&aux.join[i], cudaEventDisableTiming) == cudaSuccess;
+        }
+        ok = ok && cudaEventCreateWithFlags(&aux.fork, cudaEventDisableTiming) == cudaSuccess;
+        if (!ok) { tg_set_error("creating the auxiliary streams failed: %s", cudaGetErrorString(cudaGetLastError())); return nullptr; }
+        dev = cur;
+    }
+    return &aux;
+}
+
 extern "C" const char* tg_status_string(tg_status_t s) {
     switch (s) {
         case TG_OK: return "TG_OK";

@@ -100,6 +100,14 @@ size_t tg_side_bytes(int64_t n_rows_bound, int64_t n_edges);
 tg_status_t tg_side_build(tg_side* s, int64_t n_rows, int64_t n_edges, const int32_t* indptr, void* ws,
                           size_t ws_bytes, cudaStream_t stream);
 
+// Auxiliary streams of the calling thread (created on first use, never destroyed) for the fork / join in tiers.cuh.
+struct tg_aux_streams {
+    cudaStream_t s[2];
+    cudaEvent_t fork, join[2];
+};
+tg_aux_streams* tg_get_aux_streams();   // nullptr + tg_last_error() on failure
+constexpr int64_t TG_FORK_MIN_EDGES = 1 << 20;
+
 static inline size_t tg_align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 // ---------------------------------------------------------------------------------------------

@@ -127,14 +127,19 @@ __device__ __forceinline__ void tg_run_edges_pipe(Op& op, float (&st)[Op::NS1], 
     }
 }
 
-// Warp tier: one warp per item {row, begin, end, slot}.
-template <class Op, int U, int MIN_CTAS>
-__global__ void __launch_bounds__(TG_CTA_THREADS, MIN_CTAS) tg_warp_kernel(typename Op::Params p, const int4* __restrict__ items,
+// Warp tier: one warp per item {row, begin, end, slot}.  The warps of a CTA are independent; a CTA holds
+// TG_WARP_CTA_WARPS of them (its registers are released only when its slowest warp ends, so smaller is better
+// for the tail) and MIN_CTAS_256 * 8 / TG_WARP_CTA_WARPS such CTAs are resident per SM.
+#ifndef TG_WARP_CTA_WARPS
+#define TG_WARP_CTA_WARPS 1
+#endif
+template <class Op, int U, int MIN_CTAS_256>
+__global__ void __launch_bounds__(TG_WARP_CTA_WARPS * 32, MIN_CTAS_256 * 8 / TG_WARP_CTA_WARPS) tg_warp_kernel(typename Op::Params p, const int4* __restrict__ items,
                                                                            const int32_t* __restrict__ indptr, int n_items) {
     using Tr = typename Op::Tr;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int g = lane / Tr::LPR;
-    const int idx = blockIdx.x * TG_CTA_WARPS + warp;
+    const int idx = blockIdx.x * TG_WARP_CTA_WARPS + warp;
     if (idx >= n_items) return;
     const int4 it = items[idx];
     Op op(p, lane % Tr::LPR);
@@ -153,14 +158,17 @@ __global__ void __launch_bounds__(TG_CTA_THREADS, MIN_CTAS) tg_warp_kernel(typen
     }
 }
 
-// Group tier: one group per record {row, begin, end, 0}.
+// Group tier: one group per record {row, begin, end, 0}; TG_GROUP_CTA_WARPS independent warps per CTA.
+#ifndef TG_GROUP_CTA_WARPS
+#define TG_GROUP_CTA_WARPS 2
+#endif
 template <class Op, int U, int MIN_CTAS, bool PIPE>
-__global__ void __launch_bounds__(TG_CTA_THREADS, MIN_CTAS) tg_group_kernel(typename Op::Params p, const int4* __restrict__ rows,
+__global__ void __launch_bounds__(TG_GROUP_CTA_WARPS * 32, MIN_CTAS * 8 / TG_GROUP_CTA_WARPS) tg_group_kernel(typename Op::Params p, const int4* __restrict__ rows,
                                                                             int n_rows) {
     using Tr = typename Op::Tr;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int g = lane / Tr::LPR;
-    const int idx = (blockIdx.x * TG_CTA_WARPS + warp) * Tr::G + g;
+    const int idx = (blockIdx.x * TG_GROUP_CTA_WARPS + warp) * Tr::G + g;
     if (idx - g >= n_rows) return;  // the whole warp is idle
     const bool active = idx < n_rows;
     int4 it = make_int4(0, 0, 0, 0);  // an idle group re-reads row 0 and writes nothing
@@ -238,15 +246,42 @@ struct TierPolicy {
     static constexpr int U_PIPE = U_PIPE_, CTAS_PIPE = CTAS_PIPE_, U_PLAIN = U_PLAIN_, CTAS_PLAIN = CTAS_PLAIN_;
 };
 
-// Launch helper: all tiers of one side.
+// Launch helper: all tiers of one side.  The group tiers touch other rows than the warp tier: on a large side
+// they run on two auxiliary streams forked from and joined back into the caller's stream, so that each launch's
+// tail is filled by the others (the fork / join is a plain event pattern and can be captured into a CUDA graph).
 template <class Op, class Pol>
 static tg_status_t tg_launch_tiers(const typename Op::Params& p, const tg_side& s, cudaStream_t stream, const char* name) {
     using Tr = typename Op::Tr;
     if (s.n_rows == 0) return TG_OK;
+    constexpr int rows_per_cta = TG_GROUP_CTA_WARPS * Tr::G;
+    const int n_big = s.n_group_big(), n_small = s.n_group_small();
+    const bool fork = s.n_edges >= TG_FORK_MIN_EDGES && s.n_items > 0 && (n_big > 0 || n_small > 0);
+    tg_aux_streams* aux = nullptr;
+    if (fork) {
+        aux = tg_get_aux_streams();
+        if (!aux) return TG_ERR_CUDA;
+        TG_CUDA(cudaEventRecord(aux->fork, stream));
+    }
     if (s.n_items > 0) {
-        const unsigned grid = (unsigned)((s.n_items + TG_CTA_WARPS - 1) / TG_CTA_WARPS);
-        tg_warp_kernel<Op, Pol::U_PIPE, Pol::CTAS_PIPE><<<grid, TG_CTA_THREADS, 0, stream>>>(p, s.items, s.indptr, s.n_items);
+        const unsigned grid = (unsigned)((s.n_items + TG_WARP_CTA_WARPS - 1) / TG_WARP_CTA_WARPS);
+        tg_warp_kernel<Op, Pol::U_PIPE, Pol::CTAS_PIPE><<<grid, TG_WARP_CTA_WARPS * 32, 0, stream>>>(p, s.items, s.indptr, s.n_items);
         TG_LAUNCH_CHECK(name);
+    }
+    if (n_big > 0) {
+        cudaStream_t st = fork ? aux->s[0] : stream;
+        if (fork) TG_CUDA(cudaStreamWaitEvent(st, aux->fork, 0));
+        const unsigned grid = (unsigned)((n_big + rows_per_cta - 1) / rows_per_cta);
+        tg_group_kernel<Op, Pol::U_PIPE, Pol::CTAS_PIPE, true><<<grid, TG_GROUP_CTA_WARPS * 32, 0, st>>>(p, s.rows, n_big);
+        TG_LAUNCH_CHECK(name);
+        if (fork) TG_CUDA(cudaEventRecord(aux->join[0], st));
+    }
+    if (n_small > 0) {
+        cudaStream_t st = fork ? aux->s[1] : stream;
+        if (fork) TG_CUDA(cudaStreamWaitEvent(st, aux->fork, 0));
+        const unsigned grid = (unsigned)((n_small + rows_per_cta - 1) / rows_per_cta);
+        tg_group_kernel<Op, Pol::U_PLAIN, Pol::CTAS_PLAIN, false><<<grid, TG_GROUP_CTA_WARPS * 32, 0, st>>>(p, s.rows + n_big, n_small);
+        TG_LAUNCH_CHECK(name);
+        if (fork) TG_CUDA(cudaEventRecord(aux->join[1], st));
     }
     if constexpr (Op::NS > 0) {
         if (s.n_hubs > 0) {
@@ -261,17 +296,9 @@ static tg_status_t tg_launch_tiers(const typename Op::Params& p, const tg_side& 
             }
         }
     }
-    constexpr int rows_per_cta = TG_CTA_WARPS * Tr::G;
-    const int n_big = s.n_group_big(), n_small = s.n_group_small();
-    if (n_big > 0) {
-        const unsigned grid = (unsigned)((n_big + rows_per_cta - 1) / rows_per_cta);
-        tg_group_kernel<Op, Pol::U_PIPE, Pol::CTAS_PIPE, true><<<grid, TG_CTA_THREADS, 0, stream>>>(p, s.rows, n_big);
-        TG_LAUNCH_CHECK(name);
-    }
-    if (n_small > 0) {
-        const unsigned grid = (unsigned)((n_small + rows_per_cta - 1) / rows_per_cta);
-        tg_group_kernel<Op, Pol::U_PLAIN, Pol::CTAS_PLAIN, false><<<grid, TG_CTA_THREADS, 0, stream>>>(p, s.rows + n_big, n_small);
-        TG_LAUNCH_CHECK(name);
+    if (fork) {
+        if (n_big > 0) TG_CUDA(cudaStreamWaitEvent(stream, aux->join[0], 0));
+        if (n_small > 0) TG_CUDA(cudaStreamWaitEvent(stream, aux->join[1], 0));
     }
     return TG_OK;
 }
