@@ -16,7 +16,16 @@
 #ifndef TG_BWD1_CTASP
 #define TG_BWD1_CTASP 3
 #endif
-#define TG_BWD1_POLICY TG_BWD1_U, TG_BWD1_CTAS, TG_BWD1_UP, TG_BWD1_CTASP
+#ifndef TG_BWD1_UW
+#define TG_BWD1_UW TG_BWD1_U
+#endif
+#ifndef TG_BWD1_CTASW
+#define TG_BWD1_CTASW TG_BWD1_CTAS
+#endif
+#ifndef TG_BWD1_WPIPE
+#define TG_BWD1_WPIPE true
+#endif
+#define TG_BWD1_POLICY TG_BWD1_U, TG_BWD1_CTAS, TG_BWD1_UP, TG_BWD1_CTASP, TG_BWD1_UW, TG_BWD1_CTASW, TG_BWD1_WPIPE
 #ifndef TG_BWD2_U
 #define TG_BWD2_U 1
 #endif
@@ -29,7 +38,16 @@
 #ifndef TG_BWD2_CTASP
 #define TG_BWD2_CTASP 3
 #endif
-#define TG_BWD2_POLICY TG_BWD2_U, TG_BWD2_CTAS, TG_BWD2_UP, TG_BWD2_CTASP
+#ifndef TG_BWD2_UW
+#define TG_BWD2_UW TG_BWD2_U
+#endif
+#ifndef TG_BWD2_CTASW
+#define TG_BWD2_CTASW TG_BWD2_CTAS
+#endif
+#ifndef TG_BWD2_WPIPE
+#define TG_BWD2_WPIPE true
+#endif
+#define TG_BWD2_POLICY TG_BWD2_U, TG_BWD2_CTAS, TG_BWD2_UP, TG_BWD2_CTASP, TG_BWD2_UW, TG_BWD2_CTASW, TG_BWD2_WPIPE
 
 struct BwdArgs {
     const tg_block* b;

@@ -133,7 +133,7 @@ __device__ __forceinline__ void tg_run_edges_pipe(Op& op, float (&st)[Op::NS1], 
 #ifndef TG_WARP_CTA_WARPS
 #define TG_WARP_CTA_WARPS 1
 #endif
-template <class Op, int U, int MIN_CTAS_256>
+template <class Op, int U, int MIN_CTAS_256, bool PIPE>
 __global__ void __launch_bounds__(TG_WARP_CTA_WARPS * 32, MIN_CTAS_256 * 8 / TG_WARP_CTA_WARPS) tg_warp_kernel(typename Op::Params p, const int4* __restrict__ items,
                                                                            const int32_t* __restrict__ indptr, int n_items) {
     using Tr = typename Op::Tr;
@@ -150,7 +150,8 @@ __global__ void __launch_bounds__(TG_WARP_CTA_WARPS * 32, MIN_CTAS_256 * 8 / TG_
     const int trips = (n + Tr::G * U - 1) / (Tr::G * U);
     // a trip is full for every group when its last position (group G-1, edge U-1) is inside the chunk
     const int full_until = it.y + g + ((n / (Tr::G * U)) * (Tr::G * U));
-    tg_run_edges_pipe<U>(op, st, it.y + g, it.z, Tr::G, trips, full_until);
+    if constexpr (PIPE) tg_run_edges_pipe<U>(op, st, it.y + g, it.z, Tr::G, trips, full_until);
+    else tg_run_edges_plain<U>(op, st, it.y + g, it.z, Tr::G, trips);
     tg_warp_merge(op, st);
     if (lane < Tr::LPR) {
         if (it.w < 0) op.write_final(it.x, st, true);
@@ -241,9 +242,11 @@ __device__ __forceinline__ void tg_partial_load(const float* part, int slot, int
 
 // Launch policy of one operator: edges per trip (U) and minimum resident CTAs per SM for the pipelined
 // (warp tier, big group classes) and the plain (small group classes) variants.
-template <int U_PIPE_, int CTAS_PIPE_, int U_PLAIN_, int CTAS_PLAIN_>
+template <int U_PIPE_, int CTAS_PIPE_, int U_PLAIN_, int CTAS_PLAIN_, int U_WARP_ = U_PIPE_, int CTAS_WARP_ = CTAS_PIPE_, bool WARP_PIPE_ = true>
 struct TierPolicy {
     static constexpr int U_PIPE = U_PIPE_, CTAS_PIPE = CTAS_PIPE_, U_PLAIN = U_PLAIN_, CTAS_PLAIN = CTAS_PLAIN_;
+    static constexpr int U_WARP = U_WARP_, CTAS_WARP = CTAS_WARP_;   // warp tier: edges per trip, CTAs, pipelined or plain loop
+    static constexpr bool WARP_PIPE = WARP_PIPE_;
 };
 
 // Launch helper: all tiers of one side.  The group tiers touch other rows than the warp tier: on a large side
@@ -264,7 +267,7 @@ static tg_status_t tg_launch_tiers(const typename Op::Params& p, const tg_side& 
     }
     if (s.n_items > 0) {
         const unsigned grid = (unsigned)((s.n_items + TG_WARP_CTA_WARPS - 1) / TG_WARP_CTA_WARPS);
-        tg_warp_kernel<Op, Pol::U_PIPE, Pol::CTAS_PIPE><<<grid, TG_WARP_CTA_WARPS * 32, 0, stream>>>(p, s.items, s.indptr, s.n_items);
+        tg_warp_kernel<Op, Pol::U_WARP, Pol::CTAS_WARP, Pol::WARP_PIPE><<<grid, TG_WARP_CTA_WARPS * 32, 0, stream>>>(p, s.items, s.indptr, s.n_items);
         TG_LAUNCH_CHECK(name);
     }
     if (n_big > 0) {
