@@ -24,7 +24,7 @@
 // then single-chunk rows in classes of a factor sqrt(2) in length -- so that the 8 warps of a CTA finish together (the CTA's registers are
 // held until its slowest warp ends: unsorted items left 30 % of the resident warp slots idle on config 4).
 constexpr int TG_NICLS = 7;
-constexpr int TG_SK = TG_NCLS + TG_NICLS + 2;
+constexpr int TG_SK = TG_NCLS + TG_NICLS + 3;   // ... partial slots, hubs, big hubs (> TG_HUB_DIRECT chunks)
 __host__ __device__ constexpr int tg_item_class(int deg, int chunk) {
     if (deg > chunk) return 0;
     int c = 1;   // single-chunk rows: one class per factor sqrt(2) of length (181/256 ~ 1/sqrt 2)
@@ -48,6 +48,7 @@ struct SchedIn {
             x.v[TG_NCLS + tg_item_class(deg, chunk)] = chunks;
             x.v[TG_NCLS + TG_NICLS] = chunks > 1 ? chunks : 0;
             x.v[TG_NCLS + TG_NICLS + 1] = chunks > 1;
+            x.v[TG_NCLS + TG_NICLS + 2] = chunks > TG_HUB_DIRECT;
         }
         return x;
     }
@@ -58,6 +59,7 @@ struct SchedOut {
     int4* rows;
     int4* items;
     int4* hubs;
+    int4* bighubs;
     int* max_deg;
     __device__ __forceinline__ void operator()(int64_t i, const IVec<TG_SK>& ex, const IVec<TG_SK>& x, const IVec<TG_SK>& tot) const {
         const int row = (int)i;
@@ -78,6 +80,7 @@ struct SchedOut {
                 items[base + c] = make_int4(row, cb, ce, chunks > 1 ? ex.v[TG_NCLS + TG_NICLS] + c : -1);
             }
             if (chunks > 1) hubs[ex.v[TG_NCLS + TG_NICLS + 1]] = make_int4(row, ex.v[TG_NCLS + TG_NICLS], chunks, 0);
+            if (chunks > TG_HUB_DIRECT) bighubs[ex.v[TG_NCLS + TG_NICLS + 2]] = make_int4(row, ex.v[TG_NCLS + TG_NICLS], chunks, 0);
         }
         if (e - b > 8) atomicMax(max_deg, e - b);
     }
@@ -86,10 +89,12 @@ struct SchedOut {
 // a warp-tier row (deg > TG_GROUP_MAX) has ceil(deg / chunk) <= deg / TG_CHUNK_MIN + 1 <= 2 * deg / TG_GROUP_MAX items
 static inline int64_t side_items_bound(int64_t n_edges) { return 2 * (n_edges / TG_GROUP_MAX) + 2; }
 static inline int64_t side_hubs_bound(int64_t n_edges) { return n_edges / TG_CHUNK_MIN + 1; }
+static inline int64_t side_bighubs_bound(int64_t n_edges) { return n_edges / (TG_CHUNK_MIN * TG_HUB_DIRECT) + 1; }
 
 size_t tg_side_bytes(int64_t n_rows_bound, int64_t n_edges) {
     return tg_align_up((size_t)(n_rows_bound + 1) * sizeof(int4)) + tg_align_up((size_t)side_items_bound(n_edges) * sizeof(int4)) +
-           tg_align_up((size_t)side_hubs_bound(n_edges) * sizeof(int4)) + tg_scan_bytes<TG_SK>(n_rows_bound) + 512;
+           tg_align_up((size_t)side_hubs_bound(n_edges) * sizeof(int4)) + tg_align_up((size_t)side_bighubs_bound(n_edges) * sizeof(int4)) +
+           tg_scan_bytes<TG_SK>(n_rows_bound) + 512;
 }
 
 tg_status_t tg_side_build(tg_side* s, int64_t n_rows, int64_t n_edges, const int32_t* indptr, void* ws, size_t ws_bytes,
@@ -101,6 +106,7 @@ tg_status_t tg_side_build(tg_side* s, int64_t n_rows, int64_t n_edges, const int
     s->rows = static_cast<int4*>(c.take((size_t)(n_rows + 1) * sizeof(int4)));
     s->items = static_cast<int4*>(c.take((size_t)side_items_bound(n_edges) * sizeof(int4)));
     s->hubs = static_cast<int4*>(c.take((size_t)side_hubs_bound(n_edges) * sizeof(int4)));
+    s->bighubs = static_cast<int4*>(c.take((size_t)side_bighubs_bound(n_edges) * sizeof(int4)));
     void* scan_tmp = c.take(tg_scan_bytes<TG_SK>(n_rows));
     int* totals = static_cast<int*>(c.take(256));  // IVec<TG_SK> + max_deg at [TG_SK]
     if (!c.ok()) TG_FAIL(TG_ERR_WORKSPACE, "schedule workspace too small: need %zu, have %zu", c.off, ws_bytes);
@@ -110,7 +116,7 @@ tg_status_t tg_side_build(tg_side* s, int64_t n_rows, int64_t n_edges, const int
     while (chunk < TG_CHUNK_MAX && n_edges / chunk > 148 * 16 * 4) chunk *= 2;
     s->chunk = chunk;
     SchedIn in{indptr, chunk};
-    SchedOut out{indptr, chunk, s->rows, s->items, s->hubs, totals + TG_SK};
+    SchedOut out{indptr, chunk, s->rows, s->items, s->hubs, s->bighubs, totals + TG_SK};
     TG_TRY((tg_scan<TG_SK>(n_rows, in, out, scan_tmp, reinterpret_cast<IVec<TG_SK>*>(totals), stream)));
     int h[TG_SK + 1];
     TG_CUDA(cudaMemcpyAsync(h, totals, sizeof(h), cudaMemcpyDeviceToHost, stream));
@@ -119,7 +125,8 @@ tg_status_t tg_side_build(tg_side* s, int64_t n_rows, int64_t n_edges, const int
     for (int k = 0; k < TG_NCLS; ++k) { s->n_cls[k] = h[k]; s->n_group += h[k]; }
     s->n_items = 0;
     for (int k = 0; k < TG_NICLS; ++k) s->n_items += h[TG_NCLS + k];
-    s->n_slots = h[TG_NCLS + TG_NICLS]; s->n_hubs = h[TG_NCLS + TG_NICLS + 1]; s->max_deg = h[TG_SK];
+    s->n_slots = h[TG_NCLS + TG_NICLS]; s->n_hubs = h[TG_NCLS + TG_NICLS + 1]; s->n_bighubs = h[TG_NCLS + TG_NICLS + 2];
+    s->max_deg = h[TG_SK];
     return TG_OK;
 }
 

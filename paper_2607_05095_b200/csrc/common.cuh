@@ -64,6 +64,8 @@ constexpr int TG_NCLS_SMALL = 3;    // classes 0..2 (deg <= 8) run in the high-o
 constexpr int TG_GROUP_MAX = 64;
 constexpr int TG_CHUNK_MIN = 64, TG_CHUNK_MAX = 512;
 constexpr int TG_CTA_THREADS = 256;
+constexpr int TG_HUB_DIRECT = 32;   // a hub with more chunks is merged in two levels
+constexpr int TG_HUB_SPLIT = 16;    // CTAs per big hub in the first level
 constexpr int TG_CTA_WARPS = TG_CTA_THREADS / 32;
 
 __host__ __device__ constexpr int tg_degree_class(int deg) {
@@ -76,8 +78,9 @@ struct tg_side {
     int4* rows = nullptr;      // group tier {row, begin, end, 0}: class TG_NCLS-1 first ... class 0 last
     int4* items = nullptr;     // warp tier {row, begin, end, slot}; slot < 0: the row's only chunk
     int4* hubs = nullptr;      // {row, first_slot, n_chunks, 0}
+    int4* bighubs = nullptr;   // the hubs with more than TG_HUB_DIRECT chunks again (two-level merge)
     int32_t n_cls[TG_NCLS] = {0, 0, 0, 0, 0, 0};
-    int32_t n_group = 0, n_items = 0, n_hubs = 0, n_slots = 0;
+    int32_t n_group = 0, n_items = 0, n_hubs = 0, n_bighubs = 0, n_slots = 0;
     int32_t max_deg = 0;
     int32_t chunk = TG_CHUNK_MAX;   // edges per warp item of this side
     // group-tier rows of the classes >= TG_NCLS_SMALL come first in `rows`

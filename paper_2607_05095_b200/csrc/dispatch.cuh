@@ -69,7 +69,7 @@ struct tg_carver {
 };
 
 // partial slots of one side: one per hub chunk plus the second-level slots of the split hub merge (tiers.cuh)
-static inline size_t tg_part_slots(const tg_side& s) { return (size_t)s.n_slots + (size_t)s.n_hubs * TG_HUB_SPLIT; }
+static inline size_t tg_part_slots(const tg_side& s) { return (size_t)s.n_slots + (size_t)s.n_bighubs * TG_HUB_SPLIT; }
 
 struct tg_attn_ws_sizes { size_t fwd_part, ld, dq_part, dkv_part; };
 static inline tg_attn_ws_sizes tg_attn_ws(const tg_block* b, int H, const tg_geom& g) {

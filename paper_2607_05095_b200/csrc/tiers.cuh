@@ -184,13 +184,35 @@ __global__ void __launch_bounds__(TG_GROUP_CTA_WARPS * 32, MIN_CTAS * 8 / TG_GRO
     if (active) op.write_final(it.x, st, true);
 }
 
-// Hub merge.  A hub with <= TG_HUB_DIRECT chunks is folded by one CTA: every (warp, group) takes a strided
-// subset of the hub's partial slots.  Larger hubs (a hot source row can have thousands of chunks) are folded
-// in two levels: TG_HUB_SPLIT CTAs per hub write second-level partials (slots n_slots + hub*TG_HUB_SPLIT + j),
-// then one CTA per hub folds those.  level 0: single pass for every hub (no hub above TG_HUB_DIRECT);
-// level 1: blockIdx.y = j of the split pass (small hubs are finished here by j == 0); level 2: second pass.
-constexpr int TG_HUB_DIRECT = 32;
-constexpr int TG_HUB_SPLIT = 16;
+// Hub merge.  A hub with <= TG_HUB_DIRECT chunks is folded by one warp (tg_hub_warp_kernel).  Larger hubs (a hot
+// source row can have thousands of chunks) are folded in two levels by tg_hub_kernel: TG_HUB_SPLIT CTAs per hub
+// write second-level partials (slots n_slots + hub*TG_HUB_SPLIT + j; level 1, blockIdx.y = j), then one CTA per hub
+// folds those (level 2); they run over the schedule's separate list of big hubs.
+
+// Small hubs (<= TG_HUB_DIRECT chunks -- nearly all of them: a destination of config 4 has at most 8): one WARP per
+// hub, its G groups stride over the partial slots, shuffle merge, no shared memory and no barrier.
+constexpr int TG_HUBW_WARPS = 4;
+template <class Op>
+__global__ void __launch_bounds__(TG_HUBW_WARPS * 32) tg_hub_warp_kernel(typename Op::Params p, const int4* __restrict__ hubs, int n_hubs) {
+    using Tr = typename Op::Tr;
+    static_assert(Op::NS > 0, "an operator without state has no partials");
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int g = lane / Tr::LPR;
+    const int idx = blockIdx.x * TG_HUBW_WARPS + warp;
+    if (idx >= n_hubs) return;
+    const int4 hub = hubs[idx];  // row, first_slot, n_chunks
+    if (hub.z > TG_HUB_DIRECT) return;   // folded by the two-level tg_hub_kernel
+    Op op(p, lane % Tr::LPR);
+    float st[Op::NS];
+    op.init_state(st);
+    for (int c = g; c < hub.z; c += Tr::G) {
+        float other[Op::NS];
+        op.load_partial(hub.y + c, other);
+        op.merge(st, other);
+    }
+    tg_warp_merge(op, st);
+    if (lane < Tr::LPR) op.write_final(hub.x, st, false);
+}
 
 template <class Op>
 __global__ void __launch_bounds__(TG_CTA_THREADS) tg_hub_kernel(typename Op::Params p, const int4* __restrict__ hubs, int n_slots,
@@ -200,14 +222,11 @@ __global__ void __launch_bounds__(TG_CTA_THREADS) tg_hub_kernel(typename Op::Par
     __shared__ float sm[TG_CTA_WARPS * Tr::LPR * Op::NS];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int g = lane / Tr::LPR;
-    const int4 hub = hubs[blockIdx.x];  // row, first_slot, n_chunks
-    const bool big = hub.z > TG_HUB_DIRECT;
+    const int4 hub = hubs[blockIdx.x];  // big hubs only: row, first_slot, n_chunks
     int first = hub.y, n = hub.z, start = 0, stride = 1, out_slot = -1;
     if (level == 1) {
-        if (big) { start = blockIdx.y; stride = TG_HUB_SPLIT; out_slot = n_slots + blockIdx.x * TG_HUB_SPLIT + blockIdx.y; }
-        else if (blockIdx.y != 0) return;
-    } else if (level == 2) {
-        if (!big) return;
+        start = blockIdx.y; stride = TG_HUB_SPLIT; out_slot = n_slots + blockIdx.x * TG_HUB_SPLIT + blockIdx.y;
+    } else {
         first = n_slots + blockIdx.x * TG_HUB_SPLIT; n = TG_HUB_SPLIT;
     }
     Op op(p, lane % Tr::LPR);
@@ -288,13 +307,12 @@ static tg_status_t tg_launch_tiers(const typename Op::Params& p, const tg_side& 
     }
     if constexpr (Op::NS > 0) {
         if (s.n_hubs > 0) {
-            if (s.max_deg <= TG_HUB_DIRECT * s.chunk) {
-                tg_hub_kernel<Op><<<(unsigned)s.n_hubs, TG_CTA_THREADS, 0, stream>>>(p, s.hubs, s.n_slots, 0);
+            tg_hub_warp_kernel<Op><<<(unsigned)((s.n_hubs + TG_HUBW_WARPS - 1) / TG_HUBW_WARPS), TG_HUBW_WARPS * 32, 0, stream>>>(p, s.hubs, s.n_hubs);
+            TG_LAUNCH_CHECK(name);
+            if (s.n_bighubs > 0) {
+                tg_hub_kernel<Op><<<dim3((unsigned)s.n_bighubs, TG_HUB_SPLIT), TG_CTA_THREADS, 0, stream>>>(p, s.bighubs, s.n_slots, 1);
                 TG_LAUNCH_CHECK(name);
-            } else {
-                tg_hub_kernel<Op><<<dim3((unsigned)s.n_hubs, TG_HUB_SPLIT), TG_CTA_THREADS, 0, stream>>>(p, s.hubs, s.n_slots, 1);
-                TG_LAUNCH_CHECK(name);
-                tg_hub_kernel<Op><<<(unsigned)s.n_hubs, TG_CTA_THREADS, 0, stream>>>(p, s.hubs, s.n_slots, 2);
+                tg_hub_kernel<Op><<<(unsigned)s.n_bighubs, TG_CTA_THREADS, 0, stream>>>(p, s.bighubs, s.n_slots, 2);
                 TG_LAUNCH_CHECK(name);
             }
         }
