@@ -189,6 +189,30 @@ def test_fused_bitwise_reproducible(B):
         assert np.array_equal(x, y, equal_nan=True)
 
 
+def test_fused_cuda_graph_capture_and_side_stream(B):
+    """The fused calls only enqueue (the group tiers fork onto the library's auxiliary streams and join back):
+    they can be captured into a CUDA graph on a non-default stream, and the replay gives the eager bits."""
+    w = W.config4(0, R=30000)                     # E ~ 1.5 M: large enough for the fork / join path
+    gb = gpu_block(B, w)
+    q, k, v, do = (dev(x, torch.bfloat16) for x in w.features(gb.U))
+    O, lse = B.attn_fused_fwd(gb, q, k, v, 1.0)
+    dQ, dK, dV = B.attn_fused_bwd(gb, q, k, v, O, lse, do, 1.0)
+    torch.cuda.synchronize()
+    ref = [t.clone() for t in (O, lse, dQ, dK, dV)]
+    for t in (O, lse, dQ, dK, dV):
+        t.zero_()
+    g = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    with torch.cuda.graph(g, stream=side):
+        B.attn_fused_fwd(gb, q, k, v, 1.0, out=(O, lse))
+        B.attn_fused_bwd(gb, q, k, v, O, lse, do, 1.0, out=(dQ, dK, dV))
+    for _ in range(2):
+        g.replay()
+    torch.cuda.synchronize()
+    for a, b in zip(ref, (O, lse, dQ, dK, dV)):
+        assert torch.equal(a, b)
+
+
 # ------------------------------------------------------------------------------------------------
 # unfused operators
 # ------------------------------------------------------------------------------------------------
