@@ -19,13 +19,13 @@
 #ifndef TG_BWD1_UW
 #define TG_BWD1_UW TG_BWD1_U
 #endif
-#ifndef TG_BWD1_CTASW
-#define TG_BWD1_CTASW TG_BWD1_CTAS
+#ifndef TG_BWD1_WARPSW
+#define TG_BWD1_WARPSW (8 * TG_BWD1_CTAS)
 #endif
 #ifndef TG_BWD1_WPIPE
 #define TG_BWD1_WPIPE true
 #endif
-#define TG_BWD1_POLICY TG_BWD1_U, TG_BWD1_CTAS, TG_BWD1_UP, TG_BWD1_CTASP, TG_BWD1_UW, TG_BWD1_CTASW, TG_BWD1_WPIPE
+#define TG_BWD1_POLICY TG_BWD1_U, TG_BWD1_CTAS, TG_BWD1_UP, TG_BWD1_CTASP, TG_BWD1_UW, TG_BWD1_WARPSW, TG_BWD1_WPIPE
 #ifndef TG_BWD2_U
 #define TG_BWD2_U 1
 #endif
@@ -41,13 +41,13 @@
 #ifndef TG_BWD2_UW
 #define TG_BWD2_UW TG_BWD2_U
 #endif
-#ifndef TG_BWD2_CTASW
-#define TG_BWD2_CTASW TG_BWD2_CTAS
+#ifndef TG_BWD2_WARPSW
+#define TG_BWD2_WARPSW (8 * TG_BWD2_CTAS)
 #endif
 #ifndef TG_BWD2_WPIPE
 #define TG_BWD2_WPIPE true
 #endif
-#define TG_BWD2_POLICY TG_BWD2_U, TG_BWD2_CTAS, TG_BWD2_UP, TG_BWD2_CTASP, TG_BWD2_UW, TG_BWD2_CTASW, TG_BWD2_WPIPE
+#define TG_BWD2_POLICY TG_BWD2_U, TG_BWD2_CTAS, TG_BWD2_UP, TG_BWD2_CTASP, TG_BWD2_UW, TG_BWD2_WARPSW, TG_BWD2_WPIPE
 
 struct BwdArgs {
     const tg_block* b;

@@ -15,7 +15,13 @@
 #ifndef TG_FWD_CTASP
 #define TG_FWD_CTASP 3
 #endif
-#define TG_FWD_POLICY TG_FWD_U, TG_FWD_CTAS, TG_FWD_UP, TG_FWD_CTASP
+#ifndef TG_FWD_UW
+#define TG_FWD_UW TG_FWD_U
+#endif
+#ifndef TG_FWD_WARPSW
+#define TG_FWD_WARPSW (8 * TG_FWD_CTAS)
+#endif
+#define TG_FWD_POLICY TG_FWD_U, TG_FWD_CTAS, TG_FWD_UP, TG_FWD_CTASP, TG_FWD_UW, TG_FWD_WARPSW
 
 struct FwdArgs {
     const tg_block* b;

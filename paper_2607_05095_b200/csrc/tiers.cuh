@@ -129,12 +129,12 @@ __device__ __forceinline__ void tg_run_edges_pipe(Op& op, float (&st)[Op::NS1], 
 
 // Warp tier: one warp per item {row, begin, end, slot}.  The warps of a CTA are independent; a CTA holds
 // TG_WARP_CTA_WARPS of them (its registers are released only when its slowest warp ends, so smaller is better
-// for the tail) and MIN_CTAS_256 * 8 / TG_WARP_CTA_WARPS such CTAs are resident per SM.
+// for the tail) and MIN_WARPS / TG_WARP_CTA_WARPS such CTAs are resident per SM.
 #ifndef TG_WARP_CTA_WARPS
 #define TG_WARP_CTA_WARPS 1
 #endif
-template <class Op, int U, int MIN_CTAS_256, bool PIPE>
-__global__ void __launch_bounds__(TG_WARP_CTA_WARPS * 32, MIN_CTAS_256 * 8 / TG_WARP_CTA_WARPS) tg_warp_kernel(typename Op::Params p, const int4* __restrict__ items,
+template <class Op, int U, int MIN_WARPS, bool PIPE>
+__global__ void __launch_bounds__(TG_WARP_CTA_WARPS * 32, MIN_WARPS / TG_WARP_CTA_WARPS) tg_warp_kernel(typename Op::Params p, const int4* __restrict__ items,
                                                                            const int32_t* __restrict__ indptr, int n_items) {
     using Tr = typename Op::Tr;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -261,10 +261,10 @@ __device__ __forceinline__ void tg_partial_load(const float* part, int slot, int
 
 // Launch policy of one operator: edges per trip (U) and minimum resident CTAs per SM for the pipelined
 // (warp tier, big group classes) and the plain (small group classes) variants.
-template <int U_PIPE_, int CTAS_PIPE_, int U_PLAIN_, int CTAS_PLAIN_, int U_WARP_ = U_PIPE_, int CTAS_WARP_ = CTAS_PIPE_, bool WARP_PIPE_ = true>
+template <int U_PIPE_, int CTAS_PIPE_, int U_PLAIN_, int CTAS_PLAIN_, int U_WARP_ = U_PIPE_, int WARPS_WARP_ = 8 * CTAS_PIPE_, bool WARP_PIPE_ = true>
 struct TierPolicy {
     static constexpr int U_PIPE = U_PIPE_, CTAS_PIPE = CTAS_PIPE_, U_PLAIN = U_PLAIN_, CTAS_PLAIN = CTAS_PLAIN_;
-    static constexpr int U_WARP = U_WARP_, CTAS_WARP = CTAS_WARP_;   // warp tier: edges per trip, CTAs, pipelined or plain loop
+    static constexpr int U_WARP = U_WARP_, WARPS_WARP = WARPS_WARP_;   // warp tier: edges per trip, resident warps per SM, pipelined or plain loop
     static constexpr bool WARP_PIPE = WARP_PIPE_;
 };
 
@@ -286,7 +286,7 @@ static tg_status_t tg_launch_tiers(const typename Op::Params& p, const tg_side& 
     }
     if (s.n_items > 0) {
         const unsigned grid = (unsigned)((s.n_items + TG_WARP_CTA_WARPS - 1) / TG_WARP_CTA_WARPS);
-        tg_warp_kernel<Op, Pol::U_WARP, Pol::CTAS_WARP, Pol::WARP_PIPE><<<grid, TG_WARP_CTA_WARPS * 32, 0, stream>>>(p, s.items, s.indptr, s.n_items);
+        tg_warp_kernel<Op, Pol::U_WARP, Pol::WARPS_WARP, Pol::WARP_PIPE><<<grid, TG_WARP_CTA_WARPS * 32, 0, stream>>>(p, s.items, s.indptr, s.n_items);
         TG_LAUNCH_CHECK(name);
     }
     if (n_big > 0) {
