@@ -33,6 +33,12 @@ void tg_set_error(const char* fmt, ...);
         }                                                                                          \
     } while (0)
 
+#define TG_TRY(expr)                      \
+    do {                                  \
+        tg_status_t _s = (expr);          \
+        if (_s != TG_OK) return _s;       \
+    } while (0)
+
 // process-wide count of kernels launched by the library (tg_launch_count)
 void tg_count_launch();
 

@@ -49,11 +49,6 @@ static inline tg_status_t tg_check_rows(const void* p, const char* name) {
     do {                                                                 \
         if (!(p)) TG_FAIL(TG_ERR_INVALID_ARG, "%s is null", #p);         \
     } while (0)
-#define TG_TRY(expr)                      \
-    do {                                  \
-        tg_status_t _s = (expr);          \
-        if (_s != TG_OK) return _s;       \
-    } while (0)
 
 // workspace carving
 struct tg_carver {

@@ -133,13 +133,12 @@ __device__ __forceinline__ void tg_run_edges_pipe(Op& op, float (&st)[Op::NS1], 
 #ifndef TG_WARP_CTA_WARPS
 #define TG_WARP_CTA_WARPS 1
 #endif
-template <class Op, int U, int MIN_WARPS, bool PIPE>
-__global__ void __launch_bounds__(TG_WARP_CTA_WARPS * 32, MIN_WARPS / TG_WARP_CTA_WARPS) tg_warp_kernel(typename Op::Params p, const int4* __restrict__ items,
-                                                                           const int32_t* __restrict__ indptr, int n_items) {
+template <class Op, int U, bool PIPE>
+__device__ __forceinline__ void tg_warp_body(const typename Op::Params& p, const int4* __restrict__ items,
+                                             const int32_t* __restrict__ indptr, int n_items, int idx) {
     using Tr = typename Op::Tr;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int lane = threadIdx.x & 31;
     const int g = lane / Tr::LPR;
-    const int idx = blockIdx.x * TG_WARP_CTA_WARPS + warp;
     if (idx >= n_items) return;
     const int4 it = items[idx];
     Op op(p, lane % Tr::LPR);
@@ -158,18 +157,22 @@ __global__ void __launch_bounds__(TG_WARP_CTA_WARPS * 32, MIN_WARPS / TG_WARP_CT
         else op.write_partial(it.w, st, it.y == indptr[it.x]);
     }
 }
+template <class Op, int U, int MIN_WARPS, bool PIPE>
+__global__ void __launch_bounds__(TG_WARP_CTA_WARPS * 32, MIN_WARPS / TG_WARP_CTA_WARPS) tg_warp_kernel(typename Op::Params p, const int4* __restrict__ items,
+                                                                           const int32_t* __restrict__ indptr, int n_items) {
+    tg_warp_body<Op, U, PIPE>(p, items, indptr, n_items, blockIdx.x * TG_WARP_CTA_WARPS + (threadIdx.x >> 5));
+}
 
 // Group tier: one group per record {row, begin, end, 0}; TG_GROUP_CTA_WARPS independent warps per CTA.
 #ifndef TG_GROUP_CTA_WARPS
 #define TG_GROUP_CTA_WARPS 2
 #endif
-template <class Op, int U, int MIN_CTAS, bool PIPE>
-__global__ void __launch_bounds__(TG_GROUP_CTA_WARPS * 32, MIN_CTAS * 8 / TG_GROUP_CTA_WARPS) tg_group_kernel(typename Op::Params p, const int4* __restrict__ rows,
-                                                                            int n_rows) {
+template <class Op, int U, bool PIPE>
+__device__ __forceinline__ void tg_group_body(const typename Op::Params& p, const int4* __restrict__ rows, int n_rows, int warp_idx) {
     using Tr = typename Op::Tr;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int lane = threadIdx.x & 31;
     const int g = lane / Tr::LPR;
-    const int idx = (blockIdx.x * TG_GROUP_CTA_WARPS + warp) * Tr::G + g;
+    const int idx = warp_idx * Tr::G + g;
     if (idx - g >= n_rows) return;  // the whole warp is idle
     const bool active = idx < n_rows;
     int4 it = make_int4(0, 0, 0, 0);  // an idle group re-reads row 0 and writes nothing
@@ -182,6 +185,25 @@ __global__ void __launch_bounds__(TG_GROUP_CTA_WARPS * 32, MIN_CTAS * 8 / TG_GRO
     if constexpr (PIPE) tg_run_edges_pipe<U>(op, st, it.y, it.z, 1, trips, it.y);
     else tg_run_edges_plain<U>(op, st, it.y, it.z, 1, trips);
     if (active) op.write_final(it.x, st, true);
+}
+template <class Op, int U, int MIN_CTAS, bool PIPE>
+__global__ void __launch_bounds__(TG_GROUP_CTA_WARPS * 32, MIN_CTAS * 8 / TG_GROUP_CTA_WARPS) tg_group_kernel(typename Op::Params p, const int4* __restrict__ rows,
+                                                                            int n_rows) {
+    tg_group_body<Op, U, PIPE>(p, rows, n_rows, blockIdx.x * TG_GROUP_CTA_WARPS + (threadIdx.x >> 5));
+}
+
+// Small sides (< TG_FORK_MIN_EDGES edges: the K <= 10-20 blocks of configs 1-3) are launch-latency bound: one launch
+// covers the warp tier and both group tiers, 2 independent warps per CTA, blockIdx selects the tier (largest work first).
+template <class Op, int UW, int UB, int US, bool WARP_PIPE>
+__global__ void __launch_bounds__(64, 8) tg_small_side_kernel(typename Op::Params p, const int4* __restrict__ items, const int32_t* __restrict__ indptr,
+                                                              int n_items, const int4* __restrict__ rows, int n_big, int n_small, int nb_items, int nb_big) {
+    const int warp = threadIdx.x >> 5;
+    int b = blockIdx.x;
+    if (b < nb_items) { tg_warp_body<Op, UW, WARP_PIPE>(p, items, indptr, n_items, b * 2 + warp); return; }
+    b -= nb_items;
+    if (b < nb_big) { tg_group_body<Op, UB, true>(p, rows, n_big, b * 2 + warp); return; }
+    b -= nb_big;
+    tg_group_body<Op, US, false>(p, rows + n_big, n_small, b * 2 + warp);
 }
 
 // Hub merge.  A hub with <= TG_HUB_DIRECT chunks is folded by one warp (tg_hub_warp_kernel).  Larger hubs (a hot
@@ -268,6 +290,20 @@ struct TierPolicy {
     static constexpr bool WARP_PIPE = WARP_PIPE_;
 };
 
+template <class Op>
+static tg_status_t tg_launch_hub_merge(const typename Op::Params& p, const tg_side& s, cudaStream_t stream, const char* name) {
+    if (s.n_hubs <= 0) return TG_OK;
+    tg_hub_warp_kernel<Op><<<(unsigned)((s.n_hubs + TG_HUBW_WARPS - 1) / TG_HUBW_WARPS), TG_HUBW_WARPS * 32, 0, stream>>>(p, s.hubs, s.n_hubs);
+    TG_LAUNCH_CHECK(name);
+    if (s.n_bighubs > 0) {
+        tg_hub_kernel<Op><<<dim3((unsigned)s.n_bighubs, TG_HUB_SPLIT), TG_CTA_THREADS, 0, stream>>>(p, s.bighubs, s.n_slots, 1);
+        TG_LAUNCH_CHECK(name);
+        tg_hub_kernel<Op><<<(unsigned)s.n_bighubs, TG_CTA_THREADS, 0, stream>>>(p, s.bighubs, s.n_slots, 2);
+        TG_LAUNCH_CHECK(name);
+    }
+    return TG_OK;
+}
+
 // Launch helper: all tiers of one side.  The group tiers touch other rows than the warp tier: on a large side
 // they run on two auxiliary streams forked from and joined back into the caller's stream, so that each launch's
 // tail is filled by the others (the fork / join is a plain event pattern and can be captured into a CUDA graph).
@@ -277,7 +313,17 @@ static tg_status_t tg_launch_tiers(const typename Op::Params& p, const tg_side& 
     if (s.n_rows == 0) return TG_OK;
     constexpr int rows_per_cta = TG_GROUP_CTA_WARPS * Tr::G;
     const int n_big = s.n_group_big(), n_small = s.n_group_small();
-    const bool fork = s.n_edges >= TG_FORK_MIN_EDGES && s.n_items > 0 && (n_big > 0 || n_small > 0);
+    if (s.n_edges < TG_FORK_MIN_EDGES) {
+        const int nb_items = (s.n_items + 1) / 2, nb_big = (n_big + 2 * Tr::G - 1) / (2 * Tr::G), nb_small = (n_small + 2 * Tr::G - 1) / (2 * Tr::G);
+        if (nb_items + nb_big + nb_small > 0) {
+            tg_small_side_kernel<Op, Pol::U_WARP, Pol::U_PIPE, Pol::U_PLAIN, Pol::WARP_PIPE><<<(unsigned)(nb_items + nb_big + nb_small), 64, 0, stream>>>(
+                p, s.items, s.indptr, s.n_items, s.rows, n_big, n_small, nb_items, nb_big);
+            TG_LAUNCH_CHECK(name);
+        }
+        if constexpr (Op::NS > 0) TG_TRY((tg_launch_hub_merge<Op>(p, s, stream, name)));
+        return TG_OK;
+    }
+    const bool fork = s.n_items > 0 && (n_big > 0 || n_small > 0);
     tg_aux_streams* aux = nullptr;
     if (fork) {
         aux = tg_get_aux_streams();
@@ -305,18 +351,7 @@ static tg_status_t tg_launch_tiers(const typename Op::Params& p, const tg_side& 
         TG_LAUNCH_CHECK(name);
         if (fork) TG_CUDA(cudaEventRecord(aux->join[1], st));
     }
-    if constexpr (Op::NS > 0) {
-        if (s.n_hubs > 0) {
-            tg_hub_warp_kernel<Op><<<(unsigned)((s.n_hubs + TG_HUBW_WARPS - 1) / TG_HUBW_WARPS), TG_HUBW_WARPS * 32, 0, stream>>>(p, s.hubs, s.n_hubs);
-            TG_LAUNCH_CHECK(name);
-            if (s.n_bighubs > 0) {
-                tg_hub_kernel<Op><<<dim3((unsigned)s.n_bighubs, TG_HUB_SPLIT), TG_CTA_THREADS, 0, stream>>>(p, s.bighubs, s.n_slots, 1);
-                TG_LAUNCH_CHECK(name);
-                tg_hub_kernel<Op><<<(unsigned)s.n_bighubs, TG_CTA_THREADS, 0, stream>>>(p, s.bighubs, s.n_slots, 2);
-                TG_LAUNCH_CHECK(name);
-            }
-        }
-    }
+    if constexpr (Op::NS > 0) TG_TRY((tg_launch_hub_merge<Op>(p, s, stream, name)));
     if (fork) {
         if (n_big > 0) TG_CUDA(cudaStreamWaitEvent(stream, aux->join[0], 0));
         if (n_small > 0) TG_CUDA(cudaStreamWaitEvent(stream, aux->join[1], 0));
