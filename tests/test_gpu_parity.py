@@ -189,6 +189,30 @@ def test_fused_bitwise_reproducible(B):
         assert np.array_equal(x, y, equal_nan=True)
 
 
+def test_block_from_csr_and_empty_blocks(B, oracle_mod):
+    """tg_block_from_csr wraps index arrays the caller already has (here: the oracle's); empty blocks are TG_OK."""
+    w = _hub_workload(11, 4, 32, "f32", hub_deg=3000)
+    ob = _oblock(oracle_mod, w)
+    gb = B.block_from_csr(dev(ob.indptr), dev(ob.kv_row), ob.U, dev(ob.t_indptr), dev(ob.t_edge), dev(ob.t_dst))
+    assert gb.info()["E"] == w.E and gb.info()["U"] == ob.U
+    feats = w.features(ob.U)
+    for n, g, r in zip(("O", "LSE", "dQ", "dK", "dV"), run_fused(B, gb, w, feats, 1.5), oracle_fused(oracle_mod, ob, feats, 1.5)):
+        assert_close(n, g, r, "f32")
+    # R = 3 destinations without any edge: O = 0, LSE = -inf, dQ = 0, nothing to write on the source side
+    e = B.block_build(3, dev(np.zeros(0, np.int32)), dev(np.zeros(0, np.int64)), None, None, 1)
+    q = torch.randn(3, 8, 16, device="cuda").bfloat16()
+    kv = torch.zeros(0, 8, 16, device="cuda", dtype=torch.bfloat16)
+    O, lse = B.attn_fused_fwd(e, q, kv, kv, 1.0)
+    dQ, dK, dV = B.attn_fused_bwd(e, q, kv, kv, O, lse, q, 1.0)
+    torch.cuda.synchronize()
+    assert float(O.float().abs().max()) == 0.0 and bool(torch.isneginf(lse).all()) and float(dQ.float().abs().max()) == 0.0
+    assert dK.shape[0] == 0 and dV.shape[0] == 0
+    e0 = B.block_build(0, dev(np.zeros(0, np.int32)), dev(np.zeros(0, np.int64)), None, None, 1)
+    q0 = torch.zeros(0, 8, 16, device="cuda", dtype=torch.bfloat16)
+    O0, lse0 = B.attn_fused_fwd(e0, q0, kv, kv, 1.0)
+    assert O0.shape[0] == 0 and lse0.shape[0] == 0
+
+
 def test_fused_cuda_graph_capture_and_side_stream(B):
     """The fused calls only enqueue (the group tiers fork onto the library's auxiliary streams and join back):
     they can be captured into a CUDA graph on a non-default stream, and the replay gives the eager bits."""
