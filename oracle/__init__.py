@@ -7,4 +7,4 @@ computes and which passages of PAPER.md each function follows, and ``tests/test_
 for the pins.  Parity status: every function below is pinned (none is "parity unpinned").
 """
 from .oracle import (build, num_threads, block_build, sddmm, edge_softmax_fwd, edge_softmax_bwd,  # noqa: F401
-                     aggregate_fwd, aggregate_bwd, attn_fwd, attn_bwd, OracleBlock)
+                     aggregate_fwd, aggregate_bwd, attn_fwd, attn_bwd, attn_edge_fwd, attn_edge_bwd, OracleBlock)

@@ -190,3 +190,41 @@ def attn_bwd(indptr, kv_row, Q, K, V, dO, scale=1.0):
     if rc != 0:
         raise MemoryError("ora_attn_bwd allocation failed")
     return dQ, dK, dV
+
+
+def attn_edge_fwd(indptr, kv_row, Q, K, V, Ke=None, Ve=None, scale=1.0, slope=1.0):
+    """NEXT-1: per-edge additive key/value rows + LeakyReLU on the logits; see tg_oracle.c."""
+    lib = _load()
+    Q, K, V = _f64(Q), _f64(K), _f64(V)
+    Ke = None if Ke is None else _f64(Ke)
+    Ve = None if Ve is None else _f64(Ve)
+    H, D = _dims(Q)
+    indptr, kv_row = _i32(indptr), _i32(kv_row)
+    R = len(indptr) - 1
+    O = np.zeros((R, H, D), np.float64)
+    LSE = np.zeros((R, H), np.float64)
+    lib.ora_attn_edge_fwd(C.c_int64(R), C.c_int64(H), C.c_int64(D), _p(indptr, C.c_int32), _p(kv_row, C.c_int32),
+                          _p(Q, C.c_double), _p(K, C.c_double), _p(V, C.c_double), _p(Ke, C.c_double), _p(Ve, C.c_double),
+                          C.c_double(scale), C.c_double(slope), _p(O, C.c_double), _p(LSE, C.c_double))
+    return O, LSE
+
+
+def attn_edge_bwd(indptr, kv_row, Q, K, V, Ke, Ve, dO, scale=1.0, slope=1.0):
+    lib = _load()
+    Q, K, V, dO = _f64(Q), _f64(K), _f64(V), _f64(dO)
+    Ke = None if Ke is None else _f64(Ke)
+    Ve = None if Ve is None else _f64(Ve)
+    H, D = _dims(Q)
+    U = int(K.shape[0])
+    indptr, kv_row = _i32(indptr), _i32(kv_row)
+    R, E = len(indptr) - 1, len(kv_row)
+    dQ = np.zeros((R, H, D), np.float64)
+    dK = np.zeros((U, H, D), np.float64)
+    dV = np.zeros((U, H, D), np.float64)
+    dKe = np.zeros((E, H, D), np.float64)
+    dVe = np.zeros((E, H, D), np.float64)
+    lib.ora_attn_edge_bwd(C.c_int64(R), C.c_int64(U), C.c_int64(H), C.c_int64(D), _p(indptr, C.c_int32), _p(kv_row, C.c_int32),
+                          _p(Q, C.c_double), _p(K, C.c_double), _p(V, C.c_double), _p(Ke, C.c_double), _p(Ve, C.c_double),
+                          _p(dO, C.c_double), C.c_double(scale), C.c_double(slope),
+                          _p(dQ, C.c_double), _p(dK, C.c_double), _p(dV, C.c_double), _p(dKe, C.c_double), _p(dVe, C.c_double))
+    return dQ, dK, dV, dKe, dVe

@@ -320,6 +320,113 @@ int ora_attn_bwd(int64_t R, int64_t U, int64_t H, int64_t D, const int32_t* indp
     return 0;
 }
 
+/* ------------------------------------------------------------------------------------------ */
+/* NEXT-1: the full TGAT edge term.  Temporal attention carries "temporal and   */
+/* edge information during message passing": every sampled edge adds its own   */
+/* row (time encoding / edge-feature projection) to the gathered key and value, and TGAT-style     */
+/* logits pass a LeakyReLU.  Definitions (readings R22-R23), per head h:             */
+/*   z[e,h]  = scale * <Q[v(e),h,:], K[r(e),h,:] + Ke[e,h,:]>                                      */
+/*   s[e,h]  = z > 0 ? z : slope*z            (slope = 1: no non-linearity)                         */
+/*   alpha   = softmax over N(v) of s (three plain passes);  LSE = m + ln l                        */
+/*   O[v,h,:] = sum_{N(v)} alpha[e,h] * (V[r(e),h,:] + Ve[e,h,:])                                  */
+/* Ke, Ve are [E,H,D] in CSR order and may be NULL (= 0).                                          */
+/* ------------------------------------------------------------------------------------------ */
+void ora_attn_edge_fwd(int64_t R, int64_t H, int64_t D, const int32_t* indptr, const int32_t* kv_row,
+                       const double* Q, const double* K, const double* V, const double* Ke, const double* Ve,
+                       double scale, double slope, double* O, double* LSE) {
+    int64_t F = H * D;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t v = 0; v < R; ++v) {
+        int64_t b = indptr[v], en = indptr[v + 1], n = en - b;
+        for (int64_t i = 0; i < F; ++i) O[v * F + i] = 0.0;
+        if (n == 0) { for (int64_t h = 0; h < H; ++h) LSE[v * H + h] = -INFINITY; continue; }
+        double* s = (double*)malloc(sizeof(double) * (size_t)n);
+        for (int64_t h = 0; h < H; ++h) {
+            const double* q = Q + v * F + h * D;
+            double m = -INFINITY, l = 0.0;
+            for (int64_t e = b; e < en; ++e) {
+                const double* k = K + (int64_t)kv_row[e] * F + h * D;
+                double acc = 0.0;
+                for (int64_t d = 0; d < D; ++d) acc += q[d] * (k[d] + (Ke ? Ke[e * F + h * D + d] : 0.0));
+                double z = scale * acc;
+                s[e - b] = z > 0.0 ? z : slope * z;
+                if (s[e - b] > m) m = s[e - b];
+            }
+            for (int64_t e = b; e < en; ++e) l += exp(s[e - b] - m);
+            LSE[v * H + h] = m + log(l);
+            for (int64_t e = b; e < en; ++e) {
+                double a = exp(s[e - b] - m) / l;
+                const double* x = V + (int64_t)kv_row[e] * F + h * D;
+                for (int64_t d = 0; d < D; ++d) O[v * F + h * D + d] += a * (x[d] + (Ve ? Ve[e * F + h * D + d] : 0.0));
+            }
+        }
+        free(s);
+    }
+}
+
+/*
+ * Backward of the edge term for upstream dO:
+ *   dalpha = <dO[v], V[r]+Ve[e]>; delta = sum alpha*dalpha; ds = alpha*(dalpha - delta);
+ *   dz = ds * (z > 0 ? 1 : slope);
+ *   dQ[v] = scale * sum dz*(K[r]+Ke[e]);  dKe[e] = scale*dz*Q[v];  dVe[e] = alpha*dO[v];
+ *   dK[u] = sum_{r(e)=u} dKe[e];  dV[u] = sum_{r(e)=u} dVe[e].
+ * dKe, dVe [E,H,D] are always written (they are the per-edge terms of dK, dV).
+ */
+void ora_attn_edge_bwd(int64_t R, int64_t U, int64_t H, int64_t D, const int32_t* indptr, const int32_t* kv_row,
+                       const double* Q, const double* K, const double* V, const double* Ke, const double* Ve,
+                       const double* dO, double scale, double slope,
+                       double* dQ, double* dK, double* dV, double* dKe, double* dVe) {
+    int64_t F = H * D, E = indptr[R];
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t v = 0; v < R; ++v) {
+        int64_t b = indptr[v], en = indptr[v + 1], n = en - b;
+        for (int64_t i = 0; i < F; ++i) dQ[v * F + i] = 0.0;
+        if (n == 0) continue;
+        double* z = (double*)malloc(sizeof(double) * (size_t)n * 3);
+        double *al = z + n, *da = z + 2 * n;
+        for (int64_t h = 0; h < H; ++h) {
+            const double* q = Q + v * F + h * D;
+            const double* g = dO + v * F + h * D;
+            double m = -INFINITY, l = 0.0, delta = 0.0;
+            for (int64_t e = b; e < en; ++e) {
+                const double* k = K + (int64_t)kv_row[e] * F + h * D;
+                double acc = 0.0;
+                for (int64_t d = 0; d < D; ++d) acc += q[d] * (k[d] + (Ke ? Ke[e * F + h * D + d] : 0.0));
+                z[e - b] = scale * acc;
+                double s = z[e - b] > 0.0 ? z[e - b] : slope * z[e - b];
+                if (s > m) m = s;
+            }
+            for (int64_t e = b; e < en; ++e) { double s = z[e - b] > 0.0 ? z[e - b] : slope * z[e - b]; l += exp(s - m); }
+            for (int64_t e = b; e < en; ++e) {
+                double s = z[e - b] > 0.0 ? z[e - b] : slope * z[e - b];
+                al[e - b] = exp(s - m) / l;
+                const double* x = V + (int64_t)kv_row[e] * F + h * D;
+                double t = 0.0;
+                for (int64_t d = 0; d < D; ++d) t += g[d] * (x[d] + (Ve ? Ve[e * F + h * D + d] : 0.0));
+                da[e - b] = t;
+                delta += al[e - b] * t;
+            }
+            for (int64_t e = b; e < en; ++e) {
+                double dsv = al[e - b] * (da[e - b] - delta);
+                double dz = dsv * (z[e - b] > 0.0 ? 1.0 : slope);
+                const double* k = K + (int64_t)kv_row[e] * F + h * D;
+                for (int64_t d = 0; d < D; ++d) {
+                    dQ[v * F + h * D + d] += scale * dz * (k[d] + (Ke ? Ke[e * F + h * D + d] : 0.0));
+                    dKe[e * F + h * D + d] = scale * dz * q[d];
+                    dVe[e * F + h * D + d] = al[e - b] * g[d];
+                }
+            }
+        }
+        free(z);
+    }
+    for (int64_t i = 0; i < U * F; ++i) { dK[i] = 0.0; dV[i] = 0.0; }
+    for (int64_t e = 0; e < E; ++e)      /* plain sequential sum in CSR order */
+        for (int64_t i = 0; i < F; ++i) {
+            dK[(int64_t)kv_row[e] * F + i] += dKe[e * F + i];
+            dV[(int64_t)kv_row[e] * F + i] += dVe[e * F + i];
+        }
+}
+
 int ora_num_threads(void) {
 #ifdef _OPENMP
     extern int omp_get_max_threads(void);
