@@ -206,6 +206,27 @@ TG_API tg_status_t tg_attn_fused_bwd_src(const tg_block_t* b, int H, int D, tg_d
                                          float scale, void* dK, void* dV,
                                          void* ws, size_t ws_bytes, tg_stream_t stream);
 
+/* ------------------------------------------------------------------------------------------------
+ * NEXT-1: the full TGAT edge term -- "temporal and edge information during message
+ * passing".  Every sampled edge adds its own row (time encoding / edge-feature projection)
+ * to the gathered key and value, and the logits pass a LeakyReLU (slope = 1: none):
+ *     z[e,h] = scale * <Q[v(e),h,:], K[r(e),h,:] + Ke[e,h,:]>,   s = z > 0 ? z : slope*z,
+ *     alpha  = per-(destination, head) softmax of s,   O[v,h,:] = sum alpha * (V[r(e),h,:] + Ve[e,h,:]).
+ * Ke, Ve [E, H, D] DEVICE rows in CSR order (storage dtype, 16-byte aligned, required when E > 0).
+ * Backward writes dQ [R,H,D], dK, dV [U,H,D] and the per-edge dKe, dVe [E,H,D] (dK[u], dV[u] are their sums over the
+ * edges that reference row u).  Workspaces: the sizes tg_attn_workspace_bytes returns.  Same conventions as
+ * tg_attn_fused_fwd / _bwd (async on `stream`, zero-degree destinations, error codes).
+ * ---------------------------------------------------------------------------------------------- */
+TG_API tg_status_t tg_attn_edge_fused_fwd(const tg_block_t* b, int H, int D, tg_dtype_t dtype,
+                                          const void* Q, const void* K, const void* V, const void* Ke, const void* Ve,
+                                          float scale, float slope, void* O, float* lse,
+                                          void* ws, size_t ws_bytes, tg_stream_t stream);
+TG_API tg_status_t tg_attn_edge_fused_bwd(const tg_block_t* b, int H, int D, tg_dtype_t dtype,
+                                          const void* Q, const void* K, const void* V, const void* Ke, const void* Ve,
+                                          const void* O, const float* lse, const void* dO, float scale, float slope,
+                                          void* dQ, void* dK, void* dV, void* dKe, void* dVe,
+                                          void* ws, size_t ws_bytes, tg_stream_t stream);
+
 #ifdef __cplusplus
 }
 #endif

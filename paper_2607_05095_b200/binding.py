@@ -25,6 +25,7 @@ EXPORTS = [
     "tg_block_destroy", "tg_block_info",
     "tg_sddmm", "tg_edge_softmax_fwd", "tg_edge_softmax_bwd", "tg_aggregate_fwd", "tg_aggregate_bwd",
     "tg_attn_workspace_bytes", "tg_attn_fused_fwd", "tg_attn_fused_bwd", "tg_attn_fused_bwd_dst", "tg_attn_fused_bwd_src",
+    "tg_attn_edge_fused_fwd", "tg_attn_edge_fused_bwd",
 ]
 
 
@@ -281,3 +282,27 @@ def attn_fused_bwd_src(b: Block, Q, K, V, dO, scale: float, dK, dV):
                                        C.c_float(scale), _ptr(dK), _ptr(dV), _ptr(ws), C.c_size_t(ws.numel()), _stream()),
            "tg_attn_fused_bwd_src")
     return dK, dV
+
+
+def attn_edge_fused_fwd(b: Block, Q, K, V, Ke, Ve, scale: float = 1.0, slope: float = 1.0, out=None):
+    """tg_attn_edge_fused_fwd: per-edge additive key/value rows Ke, Ve [E,H,D] (CSR order) + LeakyReLU(slope) on the logits."""
+    Q, K, V, Ke, Ve = (_rows(t, n) for t, n in ((Q, "Q"), (K, "K"), (V, "V"), (Ke, "Ke"), (Ve, "Ve")))
+    R, H, D = Q.shape
+    O, lse = out if out is not None else (torch.empty_like(Q), torch.empty(R, H, dtype=torch.float32, device=Q.device))
+    fws, _ = b.attn_workspace(H, D, Q.dtype)
+    _check(lib().tg_attn_edge_fused_fwd(b.handle, C.c_int(H), C.c_int(D), C.c_int(_dt(Q)), _ptr(Q), _ptr(K), _ptr(V), _ptr(Ke), _ptr(Ve),
+                                        C.c_float(scale), C.c_float(slope), _ptr(O), _ptr(lse), _ptr(fws), C.c_size_t(fws.numel()),
+                                        _stream()), "tg_attn_edge_fused_fwd")
+    return O, lse
+
+
+def attn_edge_fused_bwd(b: Block, Q, K, V, Ke, Ve, O, lse, dO, scale: float = 1.0, slope: float = 1.0):
+    """tg_attn_edge_fused_bwd: returns dQ, dK, dV, dKe, dVe."""
+    Q, K, V, Ke, Ve, O, dO = (_rows(t, n) for t, n in ((Q, "Q"), (K, "K"), (V, "V"), (Ke, "Ke"), (Ve, "Ve"), (O, "O"), (dO, "dO")))
+    R, H, D = Q.shape
+    dQ, dK, dV, dKe, dVe = torch.empty_like(Q), torch.empty_like(K), torch.empty_like(V), torch.empty_like(Ke), torch.empty_like(Ve)
+    _, bws = b.attn_workspace(H, D, Q.dtype)
+    _check(lib().tg_attn_edge_fused_bwd(b.handle, C.c_int(H), C.c_int(D), C.c_int(_dt(Q)), _ptr(Q), _ptr(K), _ptr(V), _ptr(Ke), _ptr(Ve),
+                                        _ptr(O), _ptr(lse), _ptr(dO), C.c_float(scale), C.c_float(slope), _ptr(dQ), _ptr(dK), _ptr(dV),
+                                        _ptr(dKe), _ptr(dVe), _ptr(bws), C.c_size_t(bws.numel()), _stream()), "tg_attn_edge_fused_bwd")
+    return dQ, dK, dV, dKe, dVe

@@ -113,6 +113,18 @@ __device__ __forceinline__ void row_load(RowReg<Tr>& r, const typename Tr::T* p,
     }
 }
 
+// widen this lane's share of a row to fp32 (element order = ownership order)
+template <class Tr>
+__device__ __forceinline__ void row_to_float(const RowReg<Tr>& r, float (&x)[Tr::NE]) {
+    if constexpr (Tr::BF16) {
+#pragma unroll
+        for (int i = 0; i < Tr::NW; ++i) { x[2 * i] = tg_bf16lo(r.w[i]); x[2 * i + 1] = tg_bf16hi(r.w[i]); }
+    } else {
+#pragma unroll
+        for (int i = 0; i < Tr::NW; ++i) x[i] = __uint_as_float(r.w[i]);
+    }
+}
+
 // head slot of element slot k for this lane (general mode; MODE_A: k itself)
 template <class Tr, int k>
 __device__ __forceinline__ float slot_pick(const float (&x)[Tr::NHL], const LanePos<Tr>& lp) {

@@ -201,7 +201,7 @@ __global__ void __launch_bounds__(64, 8) tg_small_side_kernel(typename Op::Param
     int b = blockIdx.x;
     if (b < nb_items) { tg_warp_body<Op, UW, WARP_PIPE>(p, items, indptr, n_items, b * 2 + warp); return; }
     b -= nb_items;
-    if (b < nb_big) { tg_group_body<Op, UB, true>(p, rows, n_big, b * 2 + warp); return; }
+    if (b < nb_big) { tg_group_body<Op, UB, WARP_PIPE>(p, rows, n_big, b * 2 + warp); return; }
     b -= nb_big;
     tg_group_body<Op, US, false>(p, rows + n_big, n_small, b * 2 + warp);
 }
@@ -339,7 +339,7 @@ static tg_status_t tg_launch_tiers(const typename Op::Params& p, const tg_side& 
         cudaStream_t st = fork ? aux->s[0] : stream;
         if (fork) TG_CUDA(cudaStreamWaitEvent(st, aux->fork, 0));
         const unsigned grid = (unsigned)((n_big + rows_per_cta - 1) / rows_per_cta);
-        tg_group_kernel<Op, Pol::U_PIPE, Pol::CTAS_PIPE, true><<<grid, TG_GROUP_CTA_WARPS * 32, 0, st>>>(p, s.rows, n_big);
+        tg_group_kernel<Op, Pol::U_PIPE, Pol::CTAS_PIPE, Pol::WARP_PIPE><<<grid, TG_GROUP_CTA_WARPS * 32, 0, st>>>(p, s.rows, n_big);
         TG_LAUNCH_CHECK(name);
         if (fork) TG_CUDA(cudaEventRecord(aux->join[0], st));
     }
