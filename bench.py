@@ -15,6 +15,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import subprocess
 import sys
@@ -363,6 +364,30 @@ def run_ours(args):
         torch.cuda.synchronize()
         extras["unfused_chain_ms"] = e0.elapsed_time(e1) / 3
         del s, a
+        # NEXT-1: the full TGAT edge term on the same block -- per-edge key/value rows make it the
+        # rho = 1, HBM-bound regime.  Compulsory bytes = the base step's + Ke, Ve read once by the forward and by the
+        # backward, dKe, dVe written once.
+        if w.E * w.H * w.D * eb * 4 < 24e9:
+            gen = torch.Generator(device="cuda").manual_seed(1234)
+            ke = (torch.randn(w.E, w.H, w.D, device="cuda", generator=gen) / math.sqrt(w.D)).to(d["q"].dtype)
+            ve = (torch.randn(w.E, w.H, w.D, device="cuda", generator=gen) / math.sqrt(w.D)).to(d["q"].dtype)
+            def edge_step():
+                O, lse = B.attn_edge_fused_fwd(blk, d["q"], d["k"], d["v"], ke, ve, w.scale, 0.2, out=(o["O"], o["lse"]))
+                return B.attn_edge_fused_bwd(blk, d["q"], d["k"], d["v"], ke, ve, O, lse, d["do"], w.scale, 0.2)
+            edge_step()
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(3):
+                edge_step()
+            e1.record()
+            torch.cuda.synchronize()
+            ems = e0.elapsed_time(e1) / 3
+            f_, g_ = compulsory_bytes(w.R, w.E, bb["blk"].U, w.H, w.D, eb, w.dedup_mode)
+            ebytes = f_ + g_ + 6 * w.E * w.H * w.D * eb
+            extras["edge_term"] = {"ms_per_step": ems, "edges_per_s": w.E / (ems * 1e-3), "compulsory_bytes": ebytes,
+                                   "achieved_gbs": ebytes / (ems * 1e-3) / 1e9, "frac_of_measured_copy": ebytes / (ems * 1e-3) / 1e9 / peak,
+                                   "slope": 0.2}
+            del ke, ve
     extras["kernel_ms"] = kms
     extras["schedule"] = bb["info"]
 
