@@ -193,6 +193,11 @@ TG_API tg_status_t tg_attn_fused_bwd(const tg_block_t* b, int H, int D, tg_dtype
                                      void* dQ, void* dK, void* dV,
                                      void* ws, size_t ws_bytes, tg_stream_t stream);
 
+/* Streams.  Every attention call only enqueues work.  On a block side with >= 2^20 edges part of the work is put on
+ * two library-owned auxiliary streams that are forked from `stream` and joined back into it with events before the
+ * call returns, so for the caller the call is ordered on `stream` like a single kernel, and it can be captured into a
+ * CUDA graph (stream capture follows the fork / join).  The auxiliary streams are per calling thread and device. */
+
 /* The two passes of tg_attn_fused_bwd as separate calls (tg_attn_fused_bwd = _dst then _src on one stream),
  * for callers that want to time or overlap them.  _dst: destination-major, writes dQ and the internal
  * {LSE, delta} table into `ws`; _src: source-major over the transposed CSR, reads that table from the

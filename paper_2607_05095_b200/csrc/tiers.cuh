@@ -1,13 +1,15 @@
 // tiers.cuh -- the degree-tiered driver shared by every row-gather operator.
 //
-// A CSR side is covered by up to four launches (largest work first):
-//   tg_warp_kernel   warp tier : one warp per chunk (<= tg_side::chunk edges) of a large row; its G groups stride
-//                                over the chunk's edges, states are merged by shuffles; a hub (row with
-//                                several chunks) writes an fp32 partial per chunk
-//   tg_hub_kernel    folds each hub's partials (two levels when a hub has more than TG_HUB_DIRECT chunks)
-//   tg_group_kernel  group tier: one group per row, degree classes 9..TG_GROUP_MAX (pipelined edge loop)
-//   tg_group_kernel  group tier: degree classes <= 8 (plain edge loop, small register budget so that more
-//                                rows are in flight: these rows are pure latency chains)
+// A CSR side with >= TG_FORK_MIN_EDGES edges is covered by these launches (largest work first):
+//   tg_warp_kernel      warp tier : one warp per chunk (<= tg_side::chunk edges) of a large row; its G groups stride over
+//                                   the chunk's edges, states are merged by shuffles; a hub (row with several chunks)
+//                                   writes an fp32 partial per chunk.  1-warp CTAs, items sorted longest first.
+//   tg_hub_warp_kernel  one warp per hub with <= TG_HUB_DIRECT chunks folds its partials
+//   tg_hub_kernel       two-level fold of the few big hubs (TG_HUB_SPLIT CTAs per hub, then one)
+//   tg_group_kernel x2  group tier: one group per row, degree classes 9..TG_GROUP_MAX (pipelined edge loop) and classes
+//                                   <= 8 (plain edge loop, small register budget: these rows are pure latency chains);
+//                                   both run on auxiliary streams beside the warp tier (fork / join by events)
+// A smaller side is launch-latency bound and runs the warp tier and both group tiers in ONE launch (tg_small_side_kernel).
 // Rows of one class are contiguous in the schedule, so the groups of a warp run the same number of trips.
 //
 // An operator Op supplies: Tr (RowTraits), NS (fp32 state words per lane), Params, and
