@@ -21,7 +21,10 @@
 #ifndef TG_FWD_WARPSW
 #define TG_FWD_WARPSW (8 * TG_FWD_CTAS)
 #endif
-#define TG_FWD_POLICY TG_FWD_U, TG_FWD_CTAS, TG_FWD_UP, TG_FWD_CTASP, TG_FWD_UW, TG_FWD_WARPSW
+#ifndef TG_FWD_WPIPE
+#define TG_FWD_WPIPE true
+#endif
+#define TG_FWD_POLICY TG_FWD_U, TG_FWD_CTAS, TG_FWD_UP, TG_FWD_CTASP, TG_FWD_UW, TG_FWD_WARPSW, TG_FWD_WPIPE
 
 struct FwdArgs {
     const tg_block* b;
