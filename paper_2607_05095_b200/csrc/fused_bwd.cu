@@ -84,14 +84,21 @@ struct BwdFn {
             TG_TRY((tg_launch_tiers<Op, TierPolicy<TG_BWD1_POLICY>>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst")));
         }
         if (which & 2) {
-            using Op = Bwd2Op<Tr>;
+            // wide fp32 rows: 16 words per lane (LPR 8) and a single gather buffer; the lane layout is private to a kernel
+            constexpr bool WIDE = !Tr::BF16 && Tr::F * Tr::EB >= 512;
+            using Tr2 = RowTraits<T, Tr::H, Tr::D, WIDE ? 16 : 8>;
+            using Op = Bwd2Op<Tr2>;
+            static_assert(Tr2::NE * Tr2::LPR <= Tr::NE * Tr::LPR, "the partial workspace is sized with the default layout");
             typename Op::Params p;
             p.Q = static_cast<const T*>(a.Q); p.K = static_cast<const T*>(a.K); p.V = static_cast<const T*>(a.V);
             p.dO = static_cast<const T*>(a.dO);
             p.t_dst = a.b->t_dst; p.ld = ld;
             p.dK = static_cast<T*>(a.dK); p.dV = static_cast<T*>(a.dV); p.part = dkv_part;
             p.scale = a.scale; p.scale2 = a.scale * TG_LOG2E;
-            TG_TRY((tg_launch_tiers<Op, TierPolicy<TG_BWD2_POLICY>>(p, a.b->src, a.stream, "tg_attn_fused_bwd/src")));
+            if constexpr (WIDE)
+                TG_TRY((tg_launch_tiers<Op, TierPolicy<1, 2, 1, 2, 1, 16, false>>(p, a.b->src, a.stream, "tg_attn_fused_bwd/src")));
+            else
+                TG_TRY((tg_launch_tiers<Op, TierPolicy<TG_BWD2_POLICY>>(p, a.b->src, a.stream, "tg_attn_fused_bwd/src")));
         }
         return TG_OK;
     }

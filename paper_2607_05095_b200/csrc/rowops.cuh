@@ -21,7 +21,10 @@
 #pragma once
 #include "common.cuh"
 
-template <typename T_, int H_, int D_>
+// MAXW_: 32-bit words of one gathered row a lane may hold.  8 everywhere (two gather buffers + state fit 128 registers),
+// except the source-major backward on fp32 rows of >= 512 bytes, which runs single-buffered at 16 (LPR 8 instead of 16:
+// half the per-edge overhead instructions; config 5: 8.2 -> 6.3 ms).
+template <typename T_, int H_, int D_, int MAXW_ = 8>
 struct RowTraits {
     using T = T_;
     static constexpr int H = H_, D = D_, F = H_ * D_;
@@ -35,7 +38,7 @@ struct RowTraits {
     static constexpr int pick_lpr() {
         int lpr = 8;
         while (lpr > NV) lpr /= 2;
-        while (((NV + lpr - 1) / lpr) * WV > 8 && lpr < 32) lpr *= 2;
+        while (((NV + lpr - 1) / lpr) * WV > MAXW_ && lpr < 32) lpr *= 2;
         return lpr;
     }
     static constexpr int LPR = pick_lpr();      // lanes per row
