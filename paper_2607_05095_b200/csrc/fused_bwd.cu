@@ -74,14 +74,21 @@ struct BwdFn {
         float* dkv_part = static_cast<float*>(c.take(sz.dkv_part));
         if (!c.ok()) TG_FAIL(TG_ERR_WORKSPACE, "fused bwd needs %zu workspace bytes", c.off);
         if (which & 1) {
-            using Op = Bwd1Op<Tr>;
+            // wide fp32 rows: 16 words per lane (LPR 8) and a single gather buffer, as in the source-major pass below
+            constexpr bool WIDE1 = !Tr::BF16 && Tr::F * Tr::EB >= 512;
+            using Tr1 = RowTraits<T, Tr::H, Tr::D, WIDE1 ? 16 : 8>;
+            using Op = Bwd1Op<Tr1>;
+            static_assert(Tr1::NE * Tr1::LPR <= Tr::NE * Tr::LPR, "the partial workspace is sized with the default layout");
             typename Op::Params p;
             p.Q = static_cast<const T*>(a.Q); p.K = static_cast<const T*>(a.K); p.V = static_cast<const T*>(a.V);
             p.O = static_cast<const T*>(a.O); p.dO = static_cast<const T*>(a.dO);
             p.kv = a.b->kv_row; p.lse = a.lse;
             p.dQ = static_cast<T*>(a.dQ); p.ld = ld; p.part = dq_part;
             p.scale = a.scale; p.scale2 = a.scale * TG_LOG2E;
-            TG_TRY((tg_launch_tiers<Op, TierPolicy<TG_BWD1_POLICY>>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst")));
+            if constexpr (WIDE1)
+                TG_TRY((tg_launch_tiers<Op, TierPolicy<1, 2, 1, 2, 1, 16, false>>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst")));
+            else
+                TG_TRY((tg_launch_tiers<Op, TierPolicy<TG_BWD1_POLICY>>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst")));
         }
         if (which & 2) {
             // wide fp32 rows: 16 words per lane (LPR 8) and a single gather buffer; the lane layout is private to a kernel

@@ -22,8 +22,8 @@
 #include "common.cuh"
 
 // MAXW_: 32-bit words of one gathered row a lane may hold.  8 everywhere (two gather buffers + state fit 128 registers),
-// except the source-major backward on fp32 rows of >= 512 bytes, which runs single-buffered at 16 (LPR 8 instead of 16:
-// half the per-edge overhead instructions; config 5: 8.2 -> 6.3 ms).
+// except the two backward passes on fp32 rows of >= 512 bytes, which run single-buffered at 16 (LPR 8 instead of 16:
+// half the per-edge overhead instructions; config 5: bwd_src 8.2 -> 6.3 ms, bwd_dst 7.8 -> 7.0 ms; no gain in the forward).
 template <typename T_, int H_, int D_, int MAXW_ = 8>
 struct RowTraits {
     using T = T_;
