@@ -2,7 +2,7 @@
 // (per-edge additive key / value rows + LeakyReLU on the logits).
 //   forward : one pass, FwdEOp (online softmax fused with the aggregation, four gathered rows per edge)
 //   backward: (1) Bwd1EOp, destination-major: delta, dQ, {lse2, delta} table
-//             (2) BwdEdgeOp, destination-major, stateless: dKe[e], dVe[e] rows
+//             (2) BwdEdgeOp, destination-major, stateless: dKe[e], dVe[e] rows (bf16 only; fp32 writes them in pass 1)
 //             (3) Bwd2EOp, source-major over the transposed CSR: dK, dV accumulated in fp32 from recomputed terms
 #include "dispatch.cuh"
 #include "ops_edge.cuh"
@@ -57,10 +57,12 @@ struct EdgeBwdFn {
             p.O = static_cast<const T*>(a.O); p.dO = static_cast<const T*>(a.dO);
             p.kv = a.b->kv_row; p.lse = a.lse_in;
             p.dQ = static_cast<T*>(a.dQ); p.ld = ld; p.part = dq_part;
+            p.dKe = static_cast<T*>(a.dKe); p.dVe = static_cast<T*>(a.dVe);
             p.scale = a.scale; p.scale2 = a.scale * TG_LOG2E; p.slope = a.slope;
             TG_TRY((tg_launch_tiers<Op, EdgePolicy>(p, a.b->dst, a.stream, "tg_attn_edge_fused_bwd/dst")));
         }
-        if (a.b->E > 0) {
+        if constexpr (Tr::BF16) {   // bf16: delta comes from the edges and is final only now -> separate per-edge pass
+            if (a.b->E > 0) {
             using Op = BwdEdgeOp<Tr>;
             typename Op::Params p;
             p.Q = static_cast<const T*>(a.Q); p.K = static_cast<const T*>(a.K); p.V = static_cast<const T*>(a.V);
@@ -69,6 +71,9 @@ struct EdgeBwdFn {
             p.dKe = static_cast<T*>(a.dKe); p.dVe = static_cast<T*>(a.dVe);
             p.scale = a.scale; p.scale2 = a.scale * TG_LOG2E; p.slope = a.slope;
             TG_TRY((tg_launch_tiers<Op, EdgePolicy>(p, a.b->dst, a.stream, "tg_attn_edge_fused_bwd/edge")));
+            }
+        }
+        if (a.b->E > 0) {
             using Op2 = Bwd2EOp<Tr>;
             typename Op2::Params q;
             q.Q = static_cast<const T*>(a.Q); q.K = static_cast<const T*>(a.K); q.V = static_cast<const T*>(a.V);

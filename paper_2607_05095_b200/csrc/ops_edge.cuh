@@ -136,6 +136,7 @@ struct Bwd1EOp {
         const int32_t* kv;
         const float* lse;
         T* dQ;
+        T *dKe, *dVe;   // fp32 storage only (delta is final before the sweep): the per-edge rows are written here, no extra pass
         float2* ld;
         float* part;
         float scale, scale2, slope;
@@ -205,6 +206,18 @@ struct Bwd1EOp {
                 for (int j = 0; j < NHL; ++j) c[j] = aw[j] * (da[j] - delta[j]);
                 row_axpy_heads(st, c, b[u].k, lp);
                 row_axpy_heads(st, c, b[u].ke, lp);
+                if (ok) {   // dKe[e] = scale*dz*Q[v], dVe[e] = alpha*dO[v]
+                    const size_t e = (size_t)(pos0 + u * stride);
+                    float x[Tr::NE], cs[NHL];
+#pragma unroll
+                    for (int j = 0; j < NHL; ++j) cs[j] = c[j] * p.scale;
+                    row_to_float(q, x);
+                    row_scale_heads(x, cs, lp);
+                    row_store(p.dKe + e * Tr::F, lp, x, 1.f);
+                    row_to_float(g, x);
+                    row_scale_heads(x, a, lp);
+                    row_store(p.dVe + e * Tr::F, lp, x, 1.f);
+                }
             }
         }
     }
