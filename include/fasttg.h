@@ -101,7 +101,7 @@ TG_API int tg_supported(int H, int D, tg_dtype_t dtype);
  * dedup_mode 0: identity rows (U = E, kv_row[e] = e, uniq_node[e] = nbr_node[perm[e]]; K/V are per-edge
  *               rows [E,H,D]);  dedup_mode 1: dedup by neighbour node id.
  * All index results are exact integers with exactly one correct value (bit-exact against the oracle).
- * Errors: TG_ERR_INVALID_ARG (null, R < 0, E < 0, E >= 2^31, R >= 2^31, root_idx out of range ->
+ * Errors: TG_ERR_INVALID_ARG (null, R < 0, E < 0, E or R > 2^31 - 4096, root_idx out of range ->
  *         detected on device, reported after the sync), TG_ERR_WORKSPACE, TG_ERR_CUDA.
  * The workspace must stay alive (and untouched) until tg_block_destroy: the schedules live in it.
  * ---------------------------------------------------------------------------------------------- */

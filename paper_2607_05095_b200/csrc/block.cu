@@ -300,7 +300,7 @@ static tg_status_t build_ws_layout(int64_t R, int64_t E, int dedup_mode, tg_carv
 
 extern "C" tg_status_t tg_block_workspace_bytes(int64_t R, int64_t E, int dedup_mode, size_t* bytes) {
     if (!bytes) TG_FAIL(TG_ERR_INVALID_ARG, "bytes is null");
-    if (R < 0 || E < 0 || R >= (1LL << 31) - 1 || E >= (1LL << 31) - 1) TG_FAIL(TG_ERR_INVALID_ARG, "R=%lld E=%lld out of range", (long long)R, (long long)E);
+    if (R < 0 || E < 0 || R > TG_MAX_INDEX || E > TG_MAX_INDEX) TG_FAIL(TG_ERR_INVALID_ARG, "R=%lld E=%lld out of range", (long long)R, (long long)E);
     tg_carver c(nullptr, 0);
     BuildWs w;
     TG_TRY(build_ws_layout(R, E, dedup_mode, c, &w));
@@ -320,7 +320,8 @@ extern "C" tg_status_t tg_block_from_csr(int64_t R, int64_t E, int64_t U, const 
                                          size_t workspace_bytes, tg_stream_t stream_, tg_block_t** out) {
     if (!out) TG_FAIL(TG_ERR_INVALID_ARG, "out is null");
     *out = nullptr;
-    if (R < 0 || E < 0 || U < 0 || U > E) TG_FAIL(TG_ERR_INVALID_ARG, "bad sizes R=%lld E=%lld U=%lld", (long long)R, (long long)E, (long long)U);
+    if (R < 0 || E < 0 || U < 0 || U > E || R > TG_MAX_INDEX || E > TG_MAX_INDEX)
+        TG_FAIL(TG_ERR_INVALID_ARG, "bad sizes R=%lld E=%lld U=%lld", (long long)R, (long long)E, (long long)U);
     if (!indptr) TG_FAIL(TG_ERR_INVALID_ARG, "indptr is null");
     if (E > 0 && (!kv_row || !t_indptr || !t_edge || !t_dst)) TG_FAIL(TG_ERR_INVALID_ARG, "null index array");
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
@@ -347,7 +348,7 @@ extern "C" tg_status_t tg_block_build(int64_t R, int64_t E, const int32_t* root_
     if (!out || !U_host) TG_FAIL(TG_ERR_INVALID_ARG, "out / U_host is null");
     *out = nullptr;
     *U_host = 0;
-    if (R < 0 || E < 0 || R >= (1LL << 31) - 1 || E >= (1LL << 31) - 1) TG_FAIL(TG_ERR_INVALID_ARG, "R=%lld E=%lld out of range", (long long)R, (long long)E);
+    if (R < 0 || E < 0 || R > TG_MAX_INDEX || E > TG_MAX_INDEX) TG_FAIL(TG_ERR_INVALID_ARG, "R=%lld E=%lld out of range", (long long)R, (long long)E);
     if (dedup_mode != 0 && dedup_mode != 1) TG_FAIL(TG_ERR_INVALID_ARG, "dedup_mode must be 0 or 1");
     if (!indptr || !t_indptr) TG_FAIL(TG_ERR_INVALID_ARG, "indptr / t_indptr is null");
     if (E > 0 && (!root_idx || !nbr_node || !perm || !kv_row || !uniq_node || !t_edge || !t_dst)) TG_FAIL(TG_ERR_INVALID_ARG, "null index array");

@@ -94,6 +94,9 @@ struct tg_side {
     int32_t n_group_small() const { return n_group - n_group_big(); }
 };
 
+// Largest R / E: positions are int32 and the edge loops look a few trips (<= 4 * 32 positions) past a row's end before clamping.
+constexpr int64_t TG_MAX_INDEX = (1LL << 31) - 4096;
+
 struct tg_block {
     int64_t R = 0, E = 0, U = 0;
     const int32_t* indptr = nullptr;
