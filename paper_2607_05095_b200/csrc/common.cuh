@@ -68,7 +68,10 @@ void tg_count_launch();
 constexpr int TG_NCLS = 6;          // degree classes <=2, 3-4, 5-8, 9-16, 17-32, 33-64
 constexpr int TG_NCLS_SMALL = 3;    // classes 0..2 (deg <= 8) run in the high-occupancy kernel variant
 constexpr int TG_GROUP_MAX = 64;
-constexpr int TG_CHUNK_MIN = 64, TG_CHUNK_MAX = 512;
+#ifndef TG_CHUNK_MAX_EDGES
+#define TG_CHUNK_MAX_EDGES 1024
+#endif
+constexpr int TG_CHUNK_MIN = 64, TG_CHUNK_MAX = TG_CHUNK_MAX_EDGES;
 constexpr int TG_CTA_THREADS = 256;
 constexpr int TG_HUB_DIRECT = 32;   // a hub with more chunks is merged in two levels
 constexpr int TG_HUB_SPLIT = 16;    // CTAs per big hub in the first level

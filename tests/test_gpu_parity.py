@@ -77,7 +77,7 @@ def test_block_build_bit_exact(B, oracle_mod, w, dedup):
     deg = np.diff(ob.indptr)
     assert info["dst_group_small"] == int((deg <= 8).sum()) and info["dst_group_big"] == int(((deg > 8) & (deg <= 64)).sum())
     chunk = 64
-    while chunk < 512 and w.E // chunk > 148 * 16 * 4:
+    while chunk < 1024 and w.E // chunk > 148 * 16 * 4:
         chunk *= 2
     assert info["dst_warp_items"] == int(np.ceil(deg[deg > 64] / chunk).sum())
 
