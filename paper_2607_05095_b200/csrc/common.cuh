@@ -65,9 +65,15 @@ void tg_count_launch();
 //                                      chunk ("hub") writes fp32 partials, merged by a second launch
 // Every schedule record carries {row, begin, end}: one load instead of the order -> indptr chain.
 // ---------------------------------------------------------------------------------------------
-constexpr int TG_NCLS = 6;          // degree classes <=2, 3-4, 5-8, 9-16, 17-32, 33-64
-constexpr int TG_NCLS_SMALL = 3;    // classes 0..2 (deg <= 8) run in the high-occupancy kernel variant
-constexpr int TG_GROUP_MAX = 64;
+#ifndef TG_NCLS_N
+#define TG_NCLS_N 6
+#endif
+#ifndef TG_NCLS_SMALL_N
+#define TG_NCLS_SMALL_N 3
+#endif
+constexpr int TG_NCLS = TG_NCLS_N;              // degree classes <=2, 3-4, 5-8, 9-16, 17-32, 33-64 (, 65-128)
+constexpr int TG_NCLS_SMALL = TG_NCLS_SMALL_N;  // classes 0..2 (deg <= 8) run in the high-occupancy kernel variant
+constexpr int TG_GROUP_MAX = 2 << (TG_NCLS - 1);
 #ifndef TG_CHUNK_MAX_EDGES
 #define TG_CHUNK_MAX_EDGES 1024
 #endif
@@ -78,7 +84,7 @@ constexpr int TG_HUB_SPLIT = 16;    // CTAs per big hub in the first level
 constexpr int TG_CTA_WARPS = TG_CTA_THREADS / 32;
 
 __host__ __device__ constexpr int tg_degree_class(int deg) {
-    return deg <= 2 ? 0 : deg <= 4 ? 1 : deg <= 8 ? 2 : deg <= 16 ? 3 : deg <= 32 ? 4 : 5;
+    return deg <= 2 ? 0 : deg <= 4 ? 1 : deg <= 8 ? 2 : deg <= 16 ? 3 : deg <= 32 ? 4 : deg <= 64 ? 5 : deg <= 128 ? 6 : 7;
 }
 
 struct tg_side {
@@ -88,7 +94,7 @@ struct tg_side {
     int4* items = nullptr;     // warp tier {row, begin, end, slot}; slot < 0: the row's only chunk
     int4* hubs = nullptr;      // {row, first_slot, n_chunks, 0}
     int4* bighubs = nullptr;   // the hubs with more than TG_HUB_DIRECT chunks again (two-level merge)
-    int32_t n_cls[TG_NCLS] = {0, 0, 0, 0, 0, 0};
+    int32_t n_cls[TG_NCLS] = {};
     int32_t n_group = 0, n_items = 0, n_hubs = 0, n_bighubs = 0, n_slots = 0;
     int32_t max_deg = 0;
     int32_t chunk = TG_CHUNK_MAX;   // edges per warp item of this side
