@@ -426,6 +426,34 @@ def run_ours(args):
                                    "achieved_gbs": ebytes / (ems * 1e-3) / 1e9, "frac_of_measured_copy": ebytes / (ems * 1e-3) / 1e9 / peak,
                                    "slope": 0.2}
             del ke, ve
+        # NEXT-2: SlimCache's device half on the same block -- cache lookup of the unique source ids, then
+        # reconstruction of the per-edge K rows from (transferred unique rows || resident cache) through inv_Idx = kv_row.
+        # Algorithmic bytes: n rows written, every unique row read once, the two index arrays.
+        if w.E * w.H * w.D * eb < 24e9:
+            U_ = bb["blk"].U
+            n_ids = int(bb["blk"].uniq_node.max().item()) + 1 if U_ else 1
+            slot = torch.full((n_ids,), -1, dtype=torch.int32, device="cuda")
+            deg_u = (bb["blk"].t_indptr[1:] - bb["blk"].t_indptr[:-1]).long()
+            hot = torch.argsort(deg_u, descending=True)[: U_ // 3]              # the most referenced third is "resident"
+            slot[bb["blk"].uniq_node[hot]] = torch.arange(hot.numel(), dtype=torch.int32, device="cuda")
+            cache_rows = d["k"][hot].contiguous()
+            m_, fresh_ids = B.cache_lookup(bb["blk"].uniq_node, slot)
+            fresh_rows = d["k"][(m_ >= 0).nonzero().squeeze(1)].contiguous()
+            outk = torch.empty(w.E, w.H, w.D, dtype=d["k"].dtype, device="cuda")
+            B.feature_reconstruct(bb["blk"].kv_row, m_, fresh_rows, cache_rows, out=outk)
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(3):
+                B.feature_reconstruct(bb["blk"].kv_row, m_, fresh_rows, cache_rows, out=outk)
+            e1.record()
+            torch.cuda.synchronize()
+            rms = e0.elapsed_time(e1) / 3
+            rb = w.H * w.D * eb
+            rbytes = w.E * rb + U_ * rb + 4 * w.E + 4 * U_
+            extras["slimcache_reconstruct"] = {"ms": rms, "rows": w.E, "row_bytes": rb, "unique_rows": U_, "resident_rows": int(hot.numel()),
+                                               "transferred_rows": int(fresh_ids.numel()), "algorithmic_bytes": rbytes,
+                                               "achieved_gbs": rbytes / (rms * 1e-3) / 1e9, "frac_of_measured_copy": rbytes / (rms * 1e-3) / 1e9 / peak}
+            del outk, fresh_rows, cache_rows, slot
     extras["kernel_ms"] = kms
     extras["schedule"] = bb["info"]
 

@@ -232,6 +232,30 @@ TG_API tg_status_t tg_attn_edge_fused_bwd(const tg_block_t* b, int H, int D, tg_
                                           void* dQ, void* dK, void* dV, void* dKe, void* dVe,
                                           void* ws, size_t ws_bytes, tg_stream_t stream);
 
+/* ------------------------------------------------------------------------------------------------
+ * NEXT-2: SlimCache (section 4.2).
+ *
+ * tg_cache_greedy_select -- Algorithm 1, HOST only.  `n_batches` pre-sampled mini-batches, batch k's
+ *   node ids node_ids[node_ptr[k] .. node_ptr[k+1]) and edge ids likewise (a batch counts an id once).  Picks, by
+ *   descending access frequency (ties: ascending id; node vs edge tie: the edge), ids until i + j >= alpha*(n_nodes+n_edges).
+ *   hot_nodes [>= n_nodes], hot_edges [>= n_edges] HOST outputs in selection order, counts in n_hot_nodes / n_hot_edges.
+ * tg_cache_lookup -- runtime stage: uniq_ids[U] DEVICE int64 (a block's uniq_node, or unique edge ids),
+ *   slot_of_id DEVICE int32 indexed by id (>= 0: row of the resident cache, < 0: not cached).  Writes map[U] DEVICE int32
+ *   (>= 0: position among the rows to transfer; < 0: -(cache slot) - 1) and fresh_ids [>= U] DEVICE int64, the ids to
+ *   transfer in the order of uniq_ids; *n_fresh_host = their number.  Synchronises the stream.
+ * tg_feature_reconstruct -- out[i, :] = row of occurrence i: m = map[inv_idx ? inv_idx[i] : i];
+ *   m >= 0 ? fresh_rows[m] : cache_rows[-m-1].  Rows of row_bytes bytes (multiple of 4; 16-byte vectors when the
+ *   pointers and row_bytes allow), all DEVICE.  Async on `stream`.
+ * ---------------------------------------------------------------------------------------------- */
+TG_API tg_status_t tg_cache_greedy_select(double alpha, int64_t n_batches, const int64_t* node_ptr, const int64_t* node_ids,
+                                          const int64_t* edge_ptr, const int64_t* edge_ids, int64_t n_nodes, int64_t n_edges,
+                                          int64_t* hot_nodes, int64_t* n_hot_nodes, int64_t* hot_edges, int64_t* n_hot_edges);
+TG_API tg_status_t tg_cache_lookup_workspace_bytes(int64_t U, size_t* bytes /*HOST*/);
+TG_API tg_status_t tg_cache_lookup(int64_t U, const int64_t* uniq_ids, const int32_t* slot_of_id, int32_t* map, int64_t* fresh_ids,
+                                   int64_t* n_fresh_host /*HOST*/, void* ws, size_t ws_bytes, tg_stream_t stream);
+TG_API tg_status_t tg_feature_reconstruct(int64_t n, int64_t row_bytes, const int32_t* inv_idx, const int32_t* map,
+                                          const void* fresh_rows, const void* cache_rows, void* out, tg_stream_t stream);
+
 #ifdef __cplusplus
 }
 #endif

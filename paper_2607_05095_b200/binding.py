@@ -26,6 +26,7 @@ EXPORTS = [
     "tg_sddmm", "tg_edge_softmax_fwd", "tg_edge_softmax_bwd", "tg_aggregate_fwd", "tg_aggregate_bwd",
     "tg_attn_workspace_bytes", "tg_attn_fused_fwd", "tg_attn_fused_bwd", "tg_attn_fused_bwd_dst", "tg_attn_fused_bwd_src",
     "tg_attn_edge_fused_fwd", "tg_attn_edge_fused_bwd",
+    "tg_cache_greedy_select", "tg_cache_lookup_workspace_bytes", "tg_cache_lookup", "tg_feature_reconstruct",
 ]
 
 
@@ -306,3 +307,48 @@ def attn_edge_fused_bwd(b: Block, Q, K, V, Ke, Ve, O, lse, dO, scale: float = 1.
                                         _ptr(O), _ptr(lse), _ptr(dO), C.c_float(scale), C.c_float(slope), _ptr(dQ), _ptr(dK), _ptr(dV),
                                         _ptr(dKe), _ptr(dVe), _ptr(bws), C.c_size_t(bws.numel()), _stream()), "tg_attn_edge_fused_bwd")
     return dQ, dK, dV, dKe, dVe
+
+
+def cache_greedy_select(alpha: float, batches, n_nodes: int, n_edges: int):
+    """tg_cache_greedy_select (host): batches = list of (node_id_array, edge_id_array); returns (hot_nodes, hot_edges) int64."""
+    import numpy as np
+    nptr, eptr = [0], [0]
+    for nk, ek in batches:
+        nptr.append(nptr[-1] + len(nk)); eptr.append(eptr[-1] + len(ek))
+    cat = lambda xs: np.ascontiguousarray(np.concatenate([np.asarray(x, np.int64) for x in xs]) if xs else np.zeros(0, np.int64))
+    nid, eid = cat([b[0] for b in batches]), cat([b[1] for b in batches])
+    nptr, eptr = np.array(nptr, np.int64), np.array(eptr, np.int64)
+    hn, he = np.zeros(max(n_nodes, 1), np.int64), np.zeros(max(n_edges, 1), np.int64)
+    cn, ce = C.c_int64(0), C.c_int64(0)
+    P = lambda a: a.ctypes.data_as(C.POINTER(C.c_int64))
+    _check(lib().tg_cache_greedy_select(C.c_double(alpha), C.c_int64(len(batches)), P(nptr), P(nid), P(eptr), P(eid),
+                                        C.c_int64(n_nodes), C.c_int64(n_edges), P(hn), C.byref(cn), P(he), C.byref(ce)),
+           "tg_cache_greedy_select")
+    return hn[:cn.value].copy(), he[:ce.value].copy()
+
+
+def cache_lookup(uniq_ids: torch.Tensor, slot_of_id: torch.Tensor):
+    """tg_cache_lookup: returns (map int32 [U], fresh_ids int64 [n_fresh])."""
+    U = int(uniq_ids.shape[0])
+    m = torch.empty(U, dtype=torch.int32, device=uniq_ids.device)
+    fresh = torch.empty(U, dtype=torch.int64, device=uniq_ids.device)
+    nb = C.c_size_t()
+    _check(lib().tg_cache_lookup_workspace_bytes(C.c_int64(U), C.byref(nb)), "tg_cache_lookup_workspace_bytes")
+    ws = torch.empty(nb.value, dtype=torch.uint8, device=uniq_ids.device)
+    n = C.c_int64(0)
+    _check(lib().tg_cache_lookup(C.c_int64(U), _ptr(uniq_ids.contiguous()), _ptr(slot_of_id.contiguous()), _ptr(m), _ptr(fresh), C.byref(n),
+                                 _ptr(ws), C.c_size_t(nb.value), _stream()), "tg_cache_lookup")
+    return m, fresh[:n.value]
+
+
+def feature_reconstruct(inv_idx, map_: torch.Tensor, fresh_rows: torch.Tensor, cache_rows: torch.Tensor, out: torch.Tensor | None = None):
+    """tg_feature_reconstruct: rows [n, ...] of the occurrences listed by inv_idx (None: one per map entry)."""
+    n = int(inv_idx.shape[0]) if inv_idx is not None else int(map_.shape[0])
+    fresh_rows, cache_rows = fresh_rows.contiguous(), cache_rows.contiguous()
+    tail = tuple(fresh_rows.shape[1:])
+    row_bytes = int(fresh_rows[0].numel() * fresh_rows.element_size()) if fresh_rows.shape[0] else int(cache_rows[0].numel() * cache_rows.element_size())
+    if out is None:
+        out = torch.empty((n,) + tail, dtype=fresh_rows.dtype, device=map_.device)
+    _check(lib().tg_feature_reconstruct(C.c_int64(n), C.c_int64(row_bytes), _ptr(inv_idx), _ptr(map_), _ptr(fresh_rows), _ptr(cache_rows),
+                                        _ptr(out), _stream()), "tg_feature_reconstruct")
+    return out

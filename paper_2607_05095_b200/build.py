@@ -19,7 +19,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libfasttg.so")
-SOURCES = ["api.cu", "block.cu", "fused_fwd.cu", "fused_bwd.cu", "fused_edge.cu", "unfused.cu", "softmax.cu"]
+SOURCES = ["api.cu", "block.cu", "fused_fwd.cu", "fused_bwd.cu", "fused_edge.cu", "unfused.cu", "softmax.cu", "cache.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--use_fast_math",
               "-Xcompiler", "-fPIC,-fvisibility=hidden", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
 # tuning knobs (e.g. TG_NVCC_EXTRA="-DTG_FWD_POLICY=1,3,1,4"); part of the build stamp
