@@ -122,7 +122,7 @@ def test_fused_small_blocks(B, oracle_mod, H, D, dtype):
 @pytest.mark.parametrize("dtype", ["f32", "bf16"])
 @pytest.mark.parametrize("H,D", SHAPES)
 def test_fused_all_tiers_with_hubs(B, oracle_mod, H, D, dtype):
-    """cta tier, multi-chunk destination hubs (partial (m,l,acc) merge) and a hot source row (dK/dV partial merge)."""
+    """warp tier, multi-chunk destination hubs (partial (m,l,acc) merge) and a hot source row (dK/dV partial merge)."""
     w = _hub_workload(7 + H, H, D, dtype)
     ob = _oblock(oracle_mod, w)
     gb = gpu_block(B, w)
