@@ -211,7 +211,8 @@ __global__ void __launch_bounds__(64, 8) tg_small_side_kernel(typename Op::Param
 // Hub merge.  A hub with <= TG_HUB_DIRECT chunks is folded by one warp (tg_hub_warp_kernel).  Larger hubs (a hot
 // source row can have thousands of chunks) are folded in two levels by tg_hub_kernel: TG_HUB_SPLIT CTAs per hub
 // write second-level partials (slots n_slots + hub*TG_HUB_SPLIT + j; level 1, blockIdx.y = j), then one CTA per hub
-// folds those (level 2); they run over the schedule's separate list of big hubs.
+// folds those (level 2); they run over the schedule's separate list of big hubs.  On a small (launch-bound) side one
+// CTA per hub folds everything in a single launch (level 0).
 
 // Small hubs (<= TG_HUB_DIRECT chunks -- nearly all of them: a destination of config 4 has at most 8): one WARP per
 // hub, its G groups stride over the partial slots, shuffle merge, no shared memory and no barrier.
@@ -246,11 +247,11 @@ __global__ void __launch_bounds__(TG_CTA_THREADS) tg_hub_kernel(typename Op::Par
     __shared__ float sm[TG_CTA_WARPS * Tr::LPR * Op::NS];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int g = lane / Tr::LPR;
-    const int4 hub = hubs[blockIdx.x];  // big hubs only: row, first_slot, n_chunks
-    int first = hub.y, n = hub.z, start = 0, stride = 1, out_slot = -1;
+    const int4 hub = hubs[blockIdx.x];  // row, first_slot, n_chunks (levels 1, 2: the list of big hubs)
+    int first = hub.y, n = hub.z, start = 0, stride = 1, out_slot = -1;   // level 0: one CTA folds the whole hub
     if (level == 1) {
         start = blockIdx.y; stride = TG_HUB_SPLIT; out_slot = n_slots + blockIdx.x * TG_HUB_SPLIT + blockIdx.y;
-    } else {
+    } else if (level == 2) {
         first = n_slots + blockIdx.x * TG_HUB_SPLIT; n = TG_HUB_SPLIT;
     }
     Op op(p, lane % Tr::LPR);
@@ -295,6 +296,11 @@ struct TierPolicy {
 template <class Op>
 static tg_status_t tg_launch_hub_merge(const typename Op::Params& p, const tg_side& s, cudaStream_t stream, const char* name) {
     if (s.n_hubs <= 0) return TG_OK;
+    if (s.n_edges < TG_FORK_MIN_EDGES) {   // launch-bound small side: one CTA per hub, whatever its size, in a single launch
+        tg_hub_kernel<Op><<<(unsigned)s.n_hubs, TG_CTA_THREADS, 0, stream>>>(p, s.hubs, s.n_slots, 0);
+        TG_LAUNCH_CHECK(name);
+        return TG_OK;
+    }
     tg_hub_warp_kernel<Op><<<(unsigned)((s.n_hubs + TG_HUBW_WARPS - 1) / TG_HUBW_WARPS), TG_HUBW_WARPS * 32, 0, stream>>>(p, s.hubs, s.n_hubs);
     TG_LAUNCH_CHECK(name);
     if (s.n_bighubs > 0) {
