@@ -9,6 +9,10 @@
 
 // single-buffer loops: four gathered rows per edge leave no registers for a second buffer
 using EdgePolicy = TierPolicy<1, 2, 1, 2, 1, 16, false>;
+#ifndef TG_EDGE_FWD_WARPS
+#define TG_EDGE_FWD_WARPS 24
+#endif
+using EdgeFwdPolicy = TierPolicy<1, 2, 1, 2, 1, TG_EDGE_FWD_WARPS, false>;
 
 struct EdgeArgs {
     const tg_block* b;
@@ -34,7 +38,7 @@ struct EdgeFwdFn {
         p.kv = a.b->kv_row;
         p.O = static_cast<T*>(a.Oout); p.lse = a.lse_out; p.part = static_cast<float*>(a.ws);
         p.scale2 = a.scale * TG_LOG2E; p.slope = a.slope;
-        return tg_launch_tiers<Op, EdgePolicy>(p, a.b->dst, a.stream, "tg_attn_edge_fused_fwd");
+        return tg_launch_tiers<Op, EdgeFwdPolicy>(p, a.b->dst, a.stream, "tg_attn_edge_fused_fwd");
     }
 };
 
