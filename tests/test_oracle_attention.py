@@ -378,3 +378,19 @@ def test_online_merge_associativity():
         A = sum(q[2] * math.exp(q[0] - M) for q in parts)
         np.testing.assert_allclose(A / L, ref, rtol=1e-12, atol=1e-14)
         assert abs(M + math.log(L) - ref_lse) < 1e-12
+
+
+def test_slab_decomposition_of_source_gradients(oracle_mod):
+    """dK / dV are sums over edges and a slab of complete destinations carries the block's softmax statistics:
+    adding the oracle's per-slab results in float64 reproduces the oracle on the whole block (the host-memory
+    fallback of tests/test_gpu_configs.py for config 5 rests on this)."""
+    from gpu_util import slab_source_rows
+    w = W.small_random(77, 400, 60, 150, 2, 8, shuffle=False)
+    ob = oracle_mod.block_build(w.R, w.root_idx, w.nbr_node, w.edge_id, w.ts, 1)
+    feats = w.features(ob.U)
+    q, k, v, do = feats
+    _, dK, dV = oracle_mod.attn_bwd(ob.indptr, ob.kv_row, q, k, v, do, 1.7)
+    rows = np.arange(0, ob.U, 3)
+    sK, sV = slab_source_rows(oracle_mod, ob.indptr, ob.kv_row, feats, 1.7, rows, slab_edges=700)
+    np.testing.assert_allclose(sK, dK[rows], rtol=1e-12, atol=1e-14)
+    np.testing.assert_allclose(sV, dV[rows], rtol=1e-12, atol=1e-14)
