@@ -6,5 +6,5 @@ Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
 computes and which passages of PAPER.md each function follows, and ``tests/test_oracle_*.py``
 for the pins.  Parity status: every function below and in ``cache_oracle`` is pinned (none is "parity unpinned").
 """
-from .oracle import (build, num_threads, block_build, sddmm, edge_softmax_fwd, edge_softmax_bwd,  # noqa: F401
+from .oracle import (build, num_threads, set_num_threads, block_build, sddmm, edge_softmax_fwd, edge_softmax_bwd,  # noqa: F401
                      aggregate_fwd, aggregate_bwd, attn_fwd, attn_bwd, attn_edge_fwd, attn_edge_bwd, OracleBlock)

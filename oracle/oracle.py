@@ -37,6 +37,11 @@ def num_threads() -> int:
     return int(_load().ora_num_threads())
 
 
+def set_num_threads(n: int) -> None:
+    """OpenMP thread count of the following calls (timing legs only; results do not depend on it)."""
+    _load().ora_set_num_threads(C.c_int(int(n)))
+
+
 def _p(a, ct):
     return None if a is None else a.ctypes.data_as(C.POINTER(ct))
 

@@ -435,3 +435,13 @@ int ora_num_threads(void) {
     return 1;
 #endif
 }
+
+/* thread count of the timing legs (bench.py cpu_baseline at 1 thread and at all cores); no arithmetic */
+void ora_set_num_threads(int n) {
+#ifdef _OPENMP
+    extern void omp_set_num_threads(int);
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
