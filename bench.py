@@ -392,6 +392,70 @@ def run_extras(args, B, blocks, bi_dom, extras, peak):
             del outk, fresh_rows, cache_rows, slot
 
 
+def run_next34(args, B, blocks, bi_dom, extras, peak):
+    """NEXT-4 (plain AGG through both partitionings) and NEXT-3 (device sampler), timed separately."""
+    import torch
+    bb = blocks[bi_dom]
+    w, blk, d, o = bb["w"], bb["blk"], bb["dev"], bb["out"]
+    eb = 2 if w.dtype == "bf16" else 4
+    F = w.H * w.D
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def tm(fn, n=5):
+        fn()
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(n):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n
+
+    if F % 4 == 0 and w.E * F * 4 < 24e9:
+        coo = B.block_coo_dst(blk)
+        U_ = blk.U
+        Yc, Xc = torch.empty(w.R, w.H, w.D, dtype=torch.float32, device="cuda"), torch.empty(U_, w.H, w.D, dtype=torch.float32, device="cuda")
+        dXs = torch.empty_like(d["v"])
+        res = {}
+        # algorithmic bytes: rows in once, rows out once, the index arrays each scheme needs (CSR: indptr + one index; COO: two per-edge arrays)
+        csr_f = U_ * F * eb + w.R * F * eb + 4 * w.E + 4 * (w.R + 1)
+        csr_b = w.R * F * eb + U_ * F * eb + 4 * w.E + 4 * (U_ + 1)
+        coo_f = U_ * F * eb + w.R * F * 4 + 8 * w.E
+        coo_b = w.R * F * eb + U_ * F * 4 + 8 * w.E
+        for name, fn, nb in (("csr_fwd", lambda: B.aggregate_fwd(blk, None, d["v"], out=o["O"]), csr_f),
+                             ("csr_bwd", lambda: B.aggregate_bwd(blk, None, None, d["do"], want_dw=False), csr_b),
+                             ("coo_atomic_fwd", lambda: B.aggregate_coo(blk, d["v"], coo, out=Yc), coo_f),
+                             ("coo_atomic_bwd", lambda: B.aggregate_coo(blk, d["do"], coo, backward=True, out=Xc), coo_b)):
+            ms = tm(fn)
+            res[name] = {"ms": ms, "algorithmic_bytes": nb, "achieved_gbs": nb / (ms * 1e-3) / 1e9, "frac_of_measured_copy": nb / (ms * 1e-3) / 1e9 / peak,
+                         "edges_per_s": w.E / (ms * 1e-3)}
+        res["note"] = ("plain AGG h_v = sum v_u (PAPER.md:215) on this block: CSR gather (tg_aggregate_fwd/_bwd, w = NULL, no float atomics) vs the paper's "
+                       "COO thread-per-edge red.global.add.v4.f32 (tg_aggregate_coo, PAPER.md:219-223, float32 output, zero-fill included)")
+        extras["plain_agg"] = res
+        del Yc, Xc, dXs, coo
+    if not args.no_sampler:
+        from paper_2607_05095_b200 import workloads as W
+        n_nodes, n_events, n_roots, k = 100_000, 5_000_000, 200_000, 10
+        u, v, t = W._event_stream(args.seed, 2, n_nodes, n_events)
+        ud, vd, td = (torch.from_numpy(np.ascontiguousarray(x)).cuda() for x in (u.astype(np.int64), v.astype(np.int64), t.astype(np.float32)))
+        t_build = tm(lambda: B.tcsr_build(n_nodes, ud, vd, td), 3)
+        g = B.tcsr_build(n_nodes, ud, vd, td)
+        r = np.random.default_rng(args.seed)
+        ev = r.integers(n_events // 2, n_events, n_roots)
+        rn = torch.from_numpy(np.where(r.random(n_roots) < 0.5, u[ev], v[ev]).astype(np.int64)).cuda()
+        rc = torch.from_numpy(ev.astype(np.int64)).cuda()
+        out = {}
+        for mode in ("recent", "uniform"):
+            ms = tm(lambda: B.sample_neighbors(g, rn, rc, k, mode, 1))
+            E_s = int(B.sample_neighbors(g, rn, rc, k, mode, 1)[0].numel())
+            out[mode] = {"ms": ms, "roots": n_roots, "k": k, "sampled_edges": E_s, "sampled_edges_per_s": E_s / (ms * 1e-3),
+                         "output_bytes": 24 * E_s, "host_list_bytes_not_sent": 24 * E_s}
+        out["tcsr_build"] = {"ms": t_build, "events": n_events, "nodes": n_nodes, "entries": int(g.indptr[-1].item())}
+        out["note"] = ("device-side temporal neighbour sampler (PAPER.md:311, 412) on config 2's stream: 200 000 roots drawn from the stream's second half; "
+                       "times include output allocation and the D2H of E")
+        extras["sampler"] = out
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -627,6 +691,8 @@ def run_ours(args):
         del bb["din"], bb["dout"]
 
     run_extras(args, B, blocks, bi_dom, extras, peak)
+    if not args.no_unfused:
+        run_next34(args, B, blocks, bi_dom, extras, peak)
     extras["kernel_ms"] = kms
     extras["schedule"] = blocks[bi_dom]["info"]
 
@@ -662,7 +728,8 @@ def main():
     ap.add_argument("--src-nodes", type=int, default=0, help="diagnostic (config 4): number of source nodes; not the headline workload")
     ap.add_argument("--probe-gather", action="store_true", help="diagnostic: print the measured L1 / L2 row-gather bandwidth and exit")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--no-unfused", action="store_true")
+    ap.add_argument("--no-unfused", action="store_true", help="skip the extras: unfused chain, edge term, SlimCache, plain AGG, sampler")
+    ap.add_argument("--no-sampler", action="store_true")
     args = ap.parse_args()
     if args.probe_gather:
         from paper_2607_05095_b200 import binding as B

@@ -70,8 +70,7 @@ TG_API const char* tg_status_string(tg_status_t s);
 TG_API const char* tg_last_error(void);
 TG_API int tg_version(void);
 /* Number of kernels this library has launched in the process so far (all threads, all streams):
- * the difference across a timed region is the library's launch count for it.  Library sort launches
- * inside tg_block_build (cub) are not counted. */
+ * the difference across a timed region is the library's launch count for it. */
 TG_API unsigned long long tg_launch_count(void);
 /* Diagnostic, not part of the hot path: times `iters` launches of a pure row-gather kernel (every group of 8
  * lanes reads 256-byte rows at pseudo-random indices of `table` [table_rows, 256 bytes] DEVICE, the access shape
@@ -104,6 +103,11 @@ TG_API int tg_supported(int H, int D, tg_dtype_t dtype);
  * Errors: TG_ERR_INVALID_ARG (null, R < 0, E < 0, E or R > 2^31 - 4096, root_idx out of range ->
  *         detected on device, reported after the sync), TG_ERR_WORKSPACE, TG_ERR_CUDA.
  * The workspace must stay alive (and untouched) until tg_block_destroy: the schedules live in it.
+ * Synchronisation: every launch of the build is enqueued first, then ONE device-to-host copy (flags, U, the
+ * schedules' sizes) and ONE cudaStreamSynchronize.  What the host cannot know beforehand (is root_idx sorted? how
+ * many bits do the neighbour ids need?) is speculated from the calling thread's previous build and verified after
+ * the sync; a wrong guess repeats the build once with the measured values (first call of a thread, or a workload
+ * whose id range grows).  No library sort: csrc/radix_sort.cuh.
  * ---------------------------------------------------------------------------------------------- */
 TG_API tg_status_t tg_block_workspace_bytes(int64_t R, int64_t E, int dedup_mode, size_t* bytes /*HOST*/);
 
@@ -133,6 +137,43 @@ TG_API tg_status_t tg_block_destroy(tg_block_t* b);
  * stats[0..7] = dst side {group-tier rows with degree <= 8, group-tier rows with degree 9..64, warp-tier
  * chunk items (rows with degree > 64, one per <= 512 edges), partial slots of multi-chunk rows}, src side the same. */
 TG_API tg_status_t tg_block_info(const tg_block_t* b, int64_t* R, int64_t* E, int64_t* U, int64_t stats[8]);
+
+/* ------------------------------------------------------------------------------------------------
+ * Temporal neighbour sampler on the device
+ *
+ * PAPER.md:311 "top-k recent neighbor sampling [18] with k=10" over TGL's T-CSR.  The paper samples on
+ * the CPU (section 4.4) and ships the lists over PCIe; here the lists are produced in HBM, in the
+ * form tg_block_build consumes.
+ *
+ * tg_tcsr_build: event stream -> per-node, time-ordered incidence lists.
+ *   in : u[M], v[M] int64 endpoints in [0, n_nodes), t[M] float32 event times; event i has stream index i, the stream
+ *        is in time order (ties broken by the index, readings R20, R27)
+ *   out: tc_indptr[n_nodes+1] int64; tc_nbr / tc_eid [2M] int64, tc_ts [2M] float32 (tc_indptr[n_nodes] valid entries):
+ *        node x's entries tc_indptr[x] .. tc_indptr[x+1]-1 list, in ascending event index, every event incident to x
+ *        (either direction, a self-loop once) as {other endpoint, event index, event time}
+ *   Exact integer work (one stable radix sort).  Synchronises the stream (reports out-of-range endpoints).
+ *
+ * tg_sample_neighbors: per root i = (root_node[i], root_cutoff[i]) the prior events of its node -- event index
+ *   strictly below the cutoff -- at most k of them:
+ *     mode 0: the k most recent;  mode 1: k uniformly without replacement (all if there are <= k).
+ *   Mode 1 is Floyd's algorithm (draw d = 0..k-1: t uniform in [0, n-k+d], take t unless taken, else n-k+d) on the
+ *   counter-based stream  r(seed, i, d) = SplitMix64 output number 64*i + d + 1 of `seed`,  t = high 64 bits of r * (n-k+d+1):
+ *   reproducible, the same draw for any launch shape (reading R28).
+ *   out (capacity n_roots * k each): root_idx int32 (= i), nbr_node int64, edge_id int64, ts float32 -- roots in order,
+ *   inside a root oldest first; E_host (HOST) = number of sampled edges.  A root whose node is outside [0, n_nodes)
+ *   or has no prior event contributes nothing.  1 <= k <= 64.  Synchronises the stream (returns E).
+ * ---------------------------------------------------------------------------------------------- */
+TG_API tg_status_t tg_tcsr_workspace_bytes(int64_t n_nodes, int64_t M, size_t* bytes /*HOST*/);
+TG_API tg_status_t tg_tcsr_build(int64_t n_nodes, int64_t M, const int64_t* u, const int64_t* v, const float* t,
+                                 int64_t* tc_indptr, int64_t* tc_nbr, int64_t* tc_eid, float* tc_ts,
+                                 void* workspace, size_t workspace_bytes, tg_stream_t stream);
+TG_API tg_status_t tg_sample_workspace_bytes(int64_t n_roots, size_t* bytes /*HOST*/);
+TG_API tg_status_t tg_sample_neighbors(int mode, int k, uint64_t seed, int64_t n_roots,
+                                       const int64_t* root_node, const int64_t* root_cutoff,
+                                       int64_t n_nodes, const int64_t* tc_indptr, const int64_t* tc_nbr,
+                                       const int64_t* tc_eid, const float* tc_ts,
+                                       int32_t* root_idx, int64_t* nbr_node, int64_t* edge_id, float* ts,
+                                       int64_t* E_host /*HOST*/, void* workspace, size_t workspace_bytes, tg_stream_t stream);
 
 /* ------------------------------------------------------------------------------------------------
  * Unfused operators
@@ -167,6 +208,17 @@ TG_API tg_status_t tg_aggregate_fwd(const tg_block_t* b, int H, int D, tg_dtype_
 TG_API tg_status_t tg_aggregate_bwd(const tg_block_t* b, int H, int D, tg_dtype_t dtype,
                                     const float* w, const void* X, const void* dY,
                                     void* dX, float* dw, void* ws, size_t ws_bytes, tg_stream_t stream);
+
+/* The paper's own AGG partitioning as the measured alternative (Fig. 6(b)-III): COO, one thread per
+ * (edge, 4-element vector), one red.global.add.v4.f32 per thread.  Plain sum only (w == NULL of the calls above).
+ *   tg_block_coo_dst : coo_dst[e] = v(e), the destination of CSR edge e (int32 [E]) -- the COO row array.
+ *   tg_aggregate_coo : backward == 0:  Y[v(e)] += X[r(e)]   (X [U,H,D] in `dtype`, Y [R,H,D] float32)
+ *                      backward != 0:  Y[r(e)] += X[v(e)]   (X [R,H,D] in `dtype`, Y [U,H,D] float32)
+ *   Y is zeroed by the call and accumulated with float atomics: the result is NOT bitwise reproducible (the CSR calls
+ *   above are).  H*D must be a multiple of 4.  DESIGN.md section 15 has the measured comparison. */
+TG_API tg_status_t tg_block_coo_dst(const tg_block_t* b, int32_t* coo_dst, tg_stream_t stream);
+TG_API tg_status_t tg_aggregate_coo(const tg_block_t* b, int H, int D, tg_dtype_t dtype, int backward,
+                                    const int32_t* coo_dst, const void* X, float* Y, tg_stream_t stream);
 
 /* ------------------------------------------------------------------------------------------------
  * Fused attention (SDDMM -> ESM -> alpha-weighted AGG without materialising s or alpha)

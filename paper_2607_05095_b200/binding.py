@@ -27,6 +27,8 @@ EXPORTS = [
     "tg_attn_workspace_bytes", "tg_attn_fused_fwd", "tg_attn_fused_bwd", "tg_attn_fused_bwd_dst", "tg_attn_fused_bwd_src",
     "tg_attn_edge_fused_fwd", "tg_attn_edge_fused_bwd",
     "tg_cache_greedy_select", "tg_cache_lookup_workspace_bytes", "tg_cache_lookup", "tg_feature_reconstruct",
+    "tg_block_coo_dst", "tg_aggregate_coo",
+    "tg_tcsr_workspace_bytes", "tg_tcsr_build", "tg_sample_workspace_bytes", "tg_sample_neighbors",
 ]
 
 
@@ -352,3 +354,69 @@ def feature_reconstruct(inv_idx, map_: torch.Tensor, fresh_rows: torch.Tensor, c
     _check(lib().tg_feature_reconstruct(C.c_int64(n), C.c_int64(row_bytes), _ptr(inv_idx), _ptr(map_), _ptr(fresh_rows), _ptr(cache_rows),
                                         _ptr(out), _stream()), "tg_feature_reconstruct")
     return out
+
+
+class TCSR:
+    """Per-node, time-ordered incidence lists on the device (tg_tcsr_build)."""
+
+    def __init__(self, n_nodes, indptr, nbr, eid, ts):
+        self.n_nodes, self.indptr, self.nbr, self.eid, self.ts = n_nodes, indptr, nbr, eid, ts
+
+
+def tcsr_build(n_nodes: int, u: torch.Tensor, v: torch.Tensor, t: torch.Tensor) -> TCSR:
+    """tg_tcsr_build.  u, v int64 [M], t float32 [M] (CUDA, stream order = time order)."""
+    assert u.is_cuda and u.dtype == torch.int64 and v.dtype == torch.int64 and t.dtype == torch.float32
+    u, v, t = u.contiguous(), v.contiguous(), t.contiguous()
+    M = int(u.shape[0])
+    dev = u.device
+    indptr = torch.empty(n_nodes + 1, dtype=torch.int64, device=dev)
+    nbr = torch.empty(2 * M, dtype=torch.int64, device=dev)
+    eid = torch.empty(2 * M, dtype=torch.int64, device=dev)
+    ts = torch.empty(2 * M, dtype=torch.float32, device=dev)
+    nb = C.c_size_t()
+    _check(lib().tg_tcsr_workspace_bytes(C.c_int64(n_nodes), C.c_int64(M), C.byref(nb)), "tg_tcsr_workspace_bytes")
+    ws = torch.empty(nb.value, dtype=torch.uint8, device=dev)
+    _check(lib().tg_tcsr_build(C.c_int64(n_nodes), C.c_int64(M), _ptr(u), _ptr(v), _ptr(t), _ptr(indptr), _ptr(nbr), _ptr(eid), _ptr(ts),
+                               _ptr(ws), C.c_size_t(nb.value), _stream()), "tg_tcsr_build")
+    return TCSR(n_nodes, indptr, nbr, eid, ts)
+
+
+def sample_neighbors(g: TCSR, root_node: torch.Tensor, root_cutoff: torch.Tensor, k: int, mode: str = "recent", seed: int = 0):
+    """tg_sample_neighbors: returns tg_block_build's inputs (root_idx int32, nbr_node int64, edge_id int64, ts float32), E entries."""
+    assert root_node.is_cuda and root_node.dtype == torch.int64 and root_cutoff.dtype == torch.int64
+    root_node, root_cutoff = root_node.contiguous(), root_cutoff.contiguous()
+    n = int(root_node.shape[0])
+    dev = root_node.device
+    cap = max(n * k, 1)
+    root_idx = torch.empty(cap, dtype=torch.int32, device=dev)
+    nbr = torch.empty(cap, dtype=torch.int64, device=dev)
+    eid = torch.empty(cap, dtype=torch.int64, device=dev)
+    ts = torch.empty(cap, dtype=torch.float32, device=dev)
+    nb = C.c_size_t()
+    _check(lib().tg_sample_workspace_bytes(C.c_int64(n), C.byref(nb)), "tg_sample_workspace_bytes")
+    ws = torch.empty(nb.value, dtype=torch.uint8, device=dev)
+    E = C.c_int64(0)
+    _check(lib().tg_sample_neighbors(C.c_int({"recent": 0, "uniform": 1}[mode]), C.c_int(k), C.c_uint64(seed), C.c_int64(n), _ptr(root_node),
+                                     _ptr(root_cutoff), C.c_int64(g.n_nodes), _ptr(g.indptr), _ptr(g.nbr), _ptr(g.eid), _ptr(g.ts),
+                                     _ptr(root_idx), _ptr(nbr), _ptr(eid), _ptr(ts), C.byref(E), _ptr(ws), C.c_size_t(nb.value), _stream()),
+           "tg_sample_neighbors")
+    e = int(E.value)
+    return root_idx[:e], nbr[:e], eid[:e], ts[:e]
+
+
+def block_coo_dst(b: Block) -> torch.Tensor:
+    """tg_block_coo_dst: the COO row array (destination of every CSR edge), int32 [E]."""
+    out = torch.empty(b.E, dtype=torch.int32, device=b.indptr.device)
+    _check(lib().tg_block_coo_dst(b.handle, _ptr(out), _stream()), "tg_block_coo_dst")
+    return out
+
+
+def aggregate_coo(b: Block, X: torch.Tensor, coo_dst: torch.Tensor, backward: bool = False, out: torch.Tensor | None = None) -> torch.Tensor:
+    """tg_aggregate_coo: the paper's COO / atomic plain sum; returns float32 [R or U, H, D]."""
+    _rows(X, "X")
+    H, D = X.shape[1], X.shape[2]
+    rows = b.U if backward else b.R
+    Y = out if out is not None else torch.empty(rows, H, D, dtype=torch.float32, device=X.device)
+    _check(lib().tg_aggregate_coo(b.handle, C.c_int(H), C.c_int(D), C.c_int(_dt(X)), C.c_int(1 if backward else 0), _ptr(coo_dst),
+                                  _ptr(X), _ptr(Y), _stream()), "tg_aggregate_coo")
+    return Y

@@ -20,22 +20,25 @@ static std::atomic<unsigned long long> g_launches{0};
 void tg_count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
 extern "C" unsigned long long tg_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
+// One set of auxiliary streams per (thread, device), created on first use and kept for the life of the thread.
 tg_aux_streams* tg_get_aux_streams() {
-    static thread_local tg_aux_streams aux;
-    static thread_local int dev = -1;
+    constexpr int MAX_DEV = 64;
+    struct Slot { tg_aux_streams aux; bool ready = false; };
+    static thread_local Slot table[MAX_DEV];
     int cur = -1;
-    if (cudaGetDevice(&cur) != cudaSuccess) { tg_set_error("cudaGetDevice failed"); return nullptr; }
-    if (dev != cur) {   // first use on this thread / device
+    if (cudaGetDevice(&cur) != cudaSuccess || cur < 0 || cur >= MAX_DEV) { tg_set_error("cudaGetDevice failed or device index %d >= %d", cur, MAX_DEV); return nullptr; }
+    Slot& sl = table[cur];
+    if (!sl.ready) {
         bool ok = true;
         for (int i = 0; i < 2; ++i) {
-            ok = ok && cudaStreamCreateWithFlags(&aux.s[i], cudaStreamNonBlocking) == cudaSuccess;
-            ok = ok && cudaEventCreateWithFlags(&aux.join[i], cudaEventDisableTiming) == cudaSuccess;
+            ok = ok && cudaStreamCreateWithFlags(&sl.aux.s[i], cudaStreamNonBlocking) == cudaSuccess;
+            ok = ok && cudaEventCreateWithFlags(&sl.aux.join[i], cudaEventDisableTiming) == cudaSuccess;
         }
-        ok = ok && cudaEventCreateWithFlags(&aux.fork, cudaEventDisableTiming) == cudaSuccess;
+        ok = ok && cudaEventCreateWithFlags(&sl.aux.fork, cudaEventDisableTiming) == cudaSuccess;
         if (!ok) { tg_set_error("creating the auxiliary streams failed: %s", cudaGetErrorString(cudaGetLastError())); return nullptr; }
-        dev = cur;
+        sl.ready = true;
     }
-    return &aux;
+    return &sl.aux;
 }
 
 extern "C" const char* tg_status_string(tg_status_t s) {

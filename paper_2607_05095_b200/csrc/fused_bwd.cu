@@ -2,6 +2,7 @@
 // Pass 1, destination-major: delta, dQ (and the {lse2, delta} table).  Pass 2, source-major over the
 // transposed CSR: dK, dV by gather -- no float atomics, run-to-run bitwise reproducible.
 #include "dispatch.cuh"
+#include "ops_mma.cuh"
 
 // launch policy {edges per trip, min CTAs per SM} for the pipelined and the plain kernel variants
 #ifndef TG_BWD1_U
@@ -49,6 +50,15 @@
 #endif
 #define TG_BWD2_POLICY TG_BWD2_U, TG_BWD2_CTAS, TG_BWD2_UP, TG_BWD2_CTASP, TG_BWD2_UW, TG_BWD2_WARPSW, TG_BWD2_WPIPE
 
+// 1: bf16 rows of 256 bytes with D in {16, 32}: the warp tier takes its dot products from HMMA (ops_mma.cuh); 0 (default): FHFMA.
+// Measured on config 4 (profiles/r02_hmma_probe.md): bwd_dst 0.472 -> 0.529 ms, bwd_src 0.557 -> 0.633 ms.
+#ifndef TG_BWD1_MMA
+#define TG_BWD1_MMA 0
+#endif
+#ifndef TG_BWD2_MMA
+#define TG_BWD2_MMA 0
+#endif
+
 struct BwdArgs {
     const tg_block* b;
     const void *Q, *K, *V, *O, *dO;
@@ -87,8 +97,10 @@ struct BwdFn {
             p.scale = a.scale; p.scale2 = a.scale * TG_LOG2E;
             if constexpr (WIDE1)
                 TG_TRY((tg_launch_tiers<Op, TierPolicy<1, 2, 1, 2, 1, 16, false>>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst")));
-            else
-                TG_TRY((tg_launch_tiers<Op, TierPolicy<TG_BWD1_POLICY>>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst")));
+            else {
+                using OpW = typename tg_warp_op<Op, (TG_BWD1_MMA != 0) && MmaDotOk<Tr1>::value>::type;
+                TG_TRY((tg_launch_tiers<Op, TierPolicy<TG_BWD1_POLICY>, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst")));
+            }
         }
         if (which & 2) {
             // wide fp32 rows: 16 words per lane (LPR 8) and a single gather buffer; the lane layout is private to a kernel
@@ -104,8 +116,10 @@ struct BwdFn {
             p.scale = a.scale; p.scale2 = a.scale * TG_LOG2E;
             if constexpr (WIDE)
                 TG_TRY((tg_launch_tiers<Op, TierPolicy<1, 2, 1, 2, 1, 16, false>>(p, a.b->src, a.stream, "tg_attn_fused_bwd/src")));
-            else
-                TG_TRY((tg_launch_tiers<Op, TierPolicy<TG_BWD2_POLICY>>(p, a.b->src, a.stream, "tg_attn_fused_bwd/src")));
+            else {
+                using OpW = typename tg_warp_op<Op, (TG_BWD2_MMA != 0) && MmaDotOk<Tr2>::value>::type;
+                TG_TRY((tg_launch_tiers<Op, TierPolicy<TG_BWD2_POLICY>, OpW>(p, a.b->src, a.stream, "tg_attn_fused_bwd/src")));
+            }
         }
         return TG_OK;
     }

@@ -1,6 +1,7 @@
 // fused_fwd.cu -- tg_attn_fused_fwd: SDDMM -> edge softmax -> alpha-weighted aggregation in one pass
 // (DESIGN.md §2, §5.3).  s and alpha never reach HBM.
 #include "dispatch.cuh"
+#include "ops_mma.cuh"
 
 // launch policy {edges per trip, min CTAs per SM} for the pipelined and the plain kernel variants
 #ifndef TG_FWD_U
@@ -24,6 +25,12 @@
 #ifndef TG_FWD_WPIPE
 #define TG_FWD_WPIPE true
 #endif
+// 1: bf16 rows of 256 bytes with D in {16, 32}: the warp tier takes its logits from HMMA (ops_mma.cuh); 0 (default): FHFMA.
+// Measured on config 4 (profiles/r02_hmma_probe.md): parity green, 6 % fewer instructions, but 0.365 -> 0.396 ms: the
+// dependent HMMA chain (23 cycles each) and the block-diagonal padding cost more issue time than the FHFMA they replace.
+#ifndef TG_FWD_MMA
+#define TG_FWD_MMA 0
+#endif
 #define TG_FWD_POLICY TG_FWD_U, TG_FWD_CTAS, TG_FWD_UP, TG_FWD_CTASP, TG_FWD_UW, TG_FWD_WARPSW, TG_FWD_WPIPE
 
 struct FwdArgs {
@@ -40,6 +47,7 @@ template <class Tr>
 struct FwdFn {
     static tg_status_t run(const FwdArgs& a) {
         using Op = FwdOp<Tr>;
+        using OpW = typename tg_warp_op<Op, (TG_FWD_MMA != 0) && MmaDotOk<Tr>::value>::type;
         using T = typename Tr::T;
         typename Op::Params p;
         p.Q = static_cast<const T*>(a.Q); p.K = static_cast<const T*>(a.K); p.V = static_cast<const T*>(a.V);
@@ -48,7 +56,7 @@ struct FwdFn {
         p.lse = a.lse;
         p.part = static_cast<float*>(a.ws);
         p.scale2 = a.scale * TG_LOG2E;
-        return tg_launch_tiers<Op, TierPolicy<TG_FWD_POLICY>>(p, a.b->dst, a.stream, "tg_attn_fused_fwd");
+        return tg_launch_tiers<Op, TierPolicy<TG_FWD_POLICY>, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_fwd");
     }
 };
 

@@ -56,8 +56,10 @@ __device__ __forceinline__ IVec<K> cta_exclusive_scan(IVec<K> x, IVec<K>& total,
 }
 
 template <int K, class In>
-__global__ void __launch_bounds__(TG_SCAN_THREADS) tg_scan_reduce(int64_t n, In in, IVec<K>* tile_sums) {
+__global__ void __launch_bounds__(TG_SCAN_THREADS) tg_scan_reduce(int64_t n, const int* __restrict__ n_dev, In in, IVec<K>* tile_sums) {
     __shared__ IVec<K> sm[TG_SCAN_THREADS / 32];
+    if (n_dev) n = min(n, (int64_t)*n_dev);   // the launch was sized for the bound n; tiles past the real end sum to zero
+    if ((int64_t)blockIdx.x * TG_SCAN_TILE >= n) return;   // whole CTA; the spine stops at the real end too
     const int64_t base = (int64_t)blockIdx.x * TG_SCAN_TILE + (int64_t)threadIdx.x * TG_SCAN_ITEMS;
     IVec<K> s = ivec_zero<K>();
 #pragma unroll
@@ -69,8 +71,9 @@ __global__ void __launch_bounds__(TG_SCAN_THREADS) tg_scan_reduce(int64_t n, In 
 }
 
 template <int K>
-__global__ void __launch_bounds__(1024) tg_scan_spine(int64_t n_tiles, IVec<K>* tile_sums, IVec<K>* total_out) {
+__global__ void __launch_bounds__(1024) tg_scan_spine(int64_t n_tiles, const int* __restrict__ n_dev, IVec<K>* tile_sums, IVec<K>* total_out) {
     __shared__ IVec<K> sm[32];
+    if (n_dev) n_tiles = min(n_tiles, ((int64_t)*n_dev + TG_SCAN_TILE - 1) / TG_SCAN_TILE);   // tiles past the real end are not read by anyone
     IVec<K> carry = ivec_zero<K>();
     for (int64_t base = 0; base < n_tiles; base += 1024) {
         const int64_t i = base + threadIdx.x;
@@ -86,8 +89,10 @@ __global__ void __launch_bounds__(1024) tg_scan_spine(int64_t n_tiles, IVec<K>* 
 }
 
 template <int K, class In, class Out>
-__global__ void __launch_bounds__(TG_SCAN_THREADS) tg_scan_down(int64_t n, In in, const IVec<K>* tile_sums, const IVec<K>* total_in, Out out) {
+__global__ void __launch_bounds__(TG_SCAN_THREADS) tg_scan_down(int64_t n, const int* __restrict__ n_dev, In in, const IVec<K>* tile_sums, const IVec<K>* total_in, Out out) {
     __shared__ IVec<K> sm[TG_SCAN_THREADS / 32];
+    if (n_dev) n = min(n, (int64_t)*n_dev);
+    if ((int64_t)blockIdx.x * TG_SCAN_TILE >= n) return;   // whole CTA: no barrier is skipped by a part of it
     const int64_t base = (int64_t)blockIdx.x * TG_SCAN_TILE + (int64_t)threadIdx.x * TG_SCAN_ITEMS;
     IVec<K> x[TG_SCAN_ITEMS];
     IVec<K> s = ivec_zero<K>();
@@ -113,20 +118,21 @@ static inline size_t tg_scan_bytes(int64_t n) {
     return tg_align_up((size_t)(tiles + 1) * sizeof(IVec<K>)) + 256;
 }
 
-// `tmp` holds tg_scan_bytes<K>(n); the grand total is left at `total_dev` (device).
+// `tmp` holds tg_scan_bytes<K>(n); the grand total is left at `total_dev` (device).  n_dev (nullable): the real length
+// lives on the device (<= n, the bound the launches are sized for) -- lets a caller chain scans without a host round trip.
 template <int K, class In, class Out>
-static tg_status_t tg_scan(int64_t n, In in, Out out, void* tmp, IVec<K>* total_dev, cudaStream_t stream) {
+static tg_status_t tg_scan(int64_t n, In in, Out out, void* tmp, IVec<K>* total_dev, cudaStream_t stream, const int* n_dev = nullptr) {
     const int64_t tiles = (n + TG_SCAN_TILE - 1) / TG_SCAN_TILE;
     IVec<K>* sums = static_cast<IVec<K>*>(tmp);
     if (tiles > 0x7fffffffLL) TG_FAIL(TG_ERR_INTERNAL, "scan too large");
     if (tiles > 0) {
-        tg_scan_reduce<K, In><<<(unsigned)tiles, TG_SCAN_THREADS, 0, stream>>>(n, in, sums);
+        tg_scan_reduce<K, In><<<(unsigned)tiles, TG_SCAN_THREADS, 0, stream>>>(n, n_dev, in, sums);
         TG_LAUNCH_CHECK("tg_scan_reduce");
     }
-    tg_scan_spine<K><<<1, 1024, 0, stream>>>(tiles, sums, total_dev);
+    tg_scan_spine<K><<<1, 1024, 0, stream>>>(tiles, n_dev, sums, total_dev);
     TG_LAUNCH_CHECK("tg_scan_spine");
     if (tiles > 0) {
-        tg_scan_down<K, In, Out><<<(unsigned)tiles, TG_SCAN_THREADS, 0, stream>>>(n, in, sums, total_dev, out);
+        tg_scan_down<K, In, Out><<<(unsigned)tiles, TG_SCAN_THREADS, 0, stream>>>(n, n_dev, in, sums, total_dev, out);
         TG_LAUNCH_CHECK("tg_scan_down");
     }
     return TG_OK;

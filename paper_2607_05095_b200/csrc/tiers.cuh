@@ -21,7 +21,18 @@
 //   write_final(row, st, first), write_partial(slot, st, first), load_partial(slot, st)
 // Every warp-wide call (compute, merge) is reached by all 32 lanes with warp-uniform trip counts.
 #pragma once
+#include <type_traits>
+
 #include "rowops.cuh"
+
+// optional operator hook: end_edges(st) runs once after a work unit's edge loop, before any merge / write (an operator
+// may keep its per-head scalars in a loop-private layout, ops_mma.cuh)
+template <class Op, class = void> struct tg_has_end_edges : std::false_type {};
+template <class Op> struct tg_has_end_edges<Op, std::void_t<decltype(&Op::end_edges)>> : std::true_type {};
+template <class Op>
+__device__ __forceinline__ void tg_end_edges(Op& op, float (&st)[Op::NS1]) {
+    if constexpr (tg_has_end_edges<Op>::value) op.end_edges(st);
+}
 
 template <class Op>
 __device__ __forceinline__ void tg_warp_merge(Op& op, float (&st)[Op::NS1]) {
@@ -153,6 +164,7 @@ __device__ __forceinline__ void tg_warp_body(const typename Op::Params& p, const
     const int full_until = it.y + g + ((n / (Tr::G * U)) * (Tr::G * U));
     if constexpr (PIPE) tg_run_edges_pipe<U>(op, st, it.y + g, it.z, Tr::G, trips, full_until);
     else tg_run_edges_plain<U>(op, st, it.y + g, it.z, Tr::G, trips);
+    tg_end_edges(op, st);
     tg_warp_merge(op, st);
     if (lane < Tr::LPR) {
         if (it.w < 0) op.write_final(it.x, st, true);
@@ -186,6 +198,7 @@ __device__ __forceinline__ void tg_group_body(const typename Op::Params& p, cons
     const int trips = __reduce_max_sync(0xffffffffu, (it.z - it.y + U - 1) / U);
     if constexpr (PIPE) tg_run_edges_pipe<U>(op, st, it.y, it.z, 1, trips, it.y);
     else tg_run_edges_plain<U>(op, st, it.y, it.z, 1, trips);
+    tg_end_edges(op, st);
     if (active) op.write_final(it.x, st, true);
 }
 template <class Op, int U, int MIN_CTAS, bool PIPE>
@@ -196,12 +209,12 @@ __global__ void __launch_bounds__(TG_GROUP_CTA_WARPS * 32, MIN_CTAS * 8 / TG_GRO
 
 // Small sides (< TG_FORK_MIN_EDGES edges: the K <= 10-20 blocks of configs 1-3) are launch-latency bound: one launch
 // covers the warp tier and both group tiers, 2 independent warps per CTA, blockIdx selects the tier (largest work first).
-template <class Op, int UW, int UB, int US, bool WARP_PIPE>
+template <class Op, class OpW, int UW, int UB, int US, bool WARP_PIPE>
 __global__ void __launch_bounds__(64, 8) tg_small_side_kernel(typename Op::Params p, const int4* __restrict__ items, const int32_t* __restrict__ indptr,
                                                               int n_items, const int4* __restrict__ rows, int n_big, int n_small, int nb_items, int nb_big) {
     const int warp = threadIdx.x >> 5;
     int b = blockIdx.x;
-    if (b < nb_items) { tg_warp_body<Op, UW, WARP_PIPE>(p, items, indptr, n_items, b * 2 + warp); return; }
+    if (b < nb_items) { tg_warp_body<OpW, UW, WARP_PIPE>(p, items, indptr, n_items, b * 2 + warp); return; }
     b -= nb_items;
     if (b < nb_big) { tg_group_body<Op, UB, WARP_PIPE>(p, rows, n_big, b * 2 + warp); return; }
     b -= nb_big;
@@ -315,8 +328,10 @@ static tg_status_t tg_launch_hub_merge(const typename Op::Params& p, const tg_si
 // Launch helper: all tiers of one side.  The group tiers touch other rows than the warp tier: on a large side
 // they run on two auxiliary streams forked from and joined back into the caller's stream, so that each launch's
 // tail is filled by the others (the fork / join is a plain event pattern and can be captured into a CUDA graph).
-template <class Op, class Pol>
+// OpW: the operator of the warp tier (same Params, same state layout outside the edge loop; e.g. the HMMA variants of ops_mma.cuh).
+template <class Op, class Pol, class OpW = Op>
 static tg_status_t tg_launch_tiers(const typename Op::Params& p, const tg_side& s, cudaStream_t stream, const char* name) {
+    static_assert(std::is_same<typename Op::Params, typename OpW::Params>::value && Op::NS == OpW::NS, "warp-tier operator must share Params and state");
     using Tr = typename Op::Tr;
     if (s.n_rows == 0) return TG_OK;
     constexpr int rows_per_cta = TG_GROUP_CTA_WARPS * Tr::G;
@@ -324,7 +339,7 @@ static tg_status_t tg_launch_tiers(const typename Op::Params& p, const tg_side& 
     if (s.n_edges < TG_FORK_MIN_EDGES) {
         const int nb_items = (s.n_items + 1) / 2, nb_big = (n_big + 2 * Tr::G - 1) / (2 * Tr::G), nb_small = (n_small + 2 * Tr::G - 1) / (2 * Tr::G);
         if (nb_items + nb_big + nb_small > 0) {
-            tg_small_side_kernel<Op, Pol::U_WARP, Pol::U_PIPE, Pol::U_PLAIN, Pol::WARP_PIPE><<<(unsigned)(nb_items + nb_big + nb_small), 64, 0, stream>>>(
+            tg_small_side_kernel<Op, OpW, Pol::U_WARP, Pol::U_PIPE, Pol::U_PLAIN, Pol::WARP_PIPE><<<(unsigned)(nb_items + nb_big + nb_small), 64, 0, stream>>>(
                 p, s.items, s.indptr, s.n_items, s.rows, n_big, n_small, nb_items, nb_big);
             TG_LAUNCH_CHECK(name);
         }
@@ -338,31 +353,39 @@ static tg_status_t tg_launch_tiers(const typename Op::Params& p, const tg_side& 
         if (!aux) return TG_ERR_CUDA;
         TG_CUDA(cudaEventRecord(aux->fork, stream));
     }
-    if (s.n_items > 0) {
-        const unsigned grid = (unsigned)((s.n_items + TG_WARP_CTA_WARPS - 1) / TG_WARP_CTA_WARPS);
-        tg_warp_kernel<Op, Pol::U_WARP, Pol::WARPS_WARP, Pol::WARP_PIPE><<<grid, TG_WARP_CTA_WARPS * 32, 0, stream>>>(p, s.items, s.indptr, s.n_items);
-        TG_LAUNCH_CHECK(name);
+    // After the fork every path joins the auxiliary streams back, error or not (an unjoined fork would invalidate a stream
+    // capture and break "the call behaves like one kernel on `stream`"): the first error is kept and returned at the end.
+    tg_status_t st = TG_OK;
+    bool forked[2] = {false, false};
+    auto launch_all = [&]() -> tg_status_t {
+        if (s.n_items > 0) {
+            const unsigned grid = (unsigned)((s.n_items + TG_WARP_CTA_WARPS - 1) / TG_WARP_CTA_WARPS);
+            tg_warp_kernel<OpW, Pol::U_WARP, Pol::WARPS_WARP, Pol::WARP_PIPE><<<grid, TG_WARP_CTA_WARPS * 32, 0, stream>>>(p, s.items, s.indptr, s.n_items);
+            TG_LAUNCH_CHECK(name);
+        }
+        if (n_big > 0) {
+            cudaStream_t sx = fork ? aux->s[0] : stream;
+            if (fork) { TG_CUDA(cudaStreamWaitEvent(sx, aux->fork, 0)); forked[0] = true; }
+            const unsigned grid = (unsigned)((n_big + rows_per_cta - 1) / rows_per_cta);
+            tg_group_kernel<Op, Pol::U_PIPE, Pol::CTAS_PIPE, Pol::WARP_PIPE><<<grid, TG_GROUP_CTA_WARPS * 32, 0, sx>>>(p, s.rows, n_big);
+            TG_LAUNCH_CHECK(name);
+        }
+        if (n_small > 0) {
+            cudaStream_t sx = fork ? aux->s[1] : stream;
+            if (fork) { TG_CUDA(cudaStreamWaitEvent(sx, aux->fork, 0)); forked[1] = true; }
+            const unsigned grid = (unsigned)((n_small + rows_per_cta - 1) / rows_per_cta);
+            tg_group_kernel<Op, Pol::U_PLAIN, Pol::CTAS_PLAIN, false><<<grid, TG_GROUP_CTA_WARPS * 32, 0, sx>>>(p, s.rows + n_big, n_small);
+            TG_LAUNCH_CHECK(name);
+        }
+        if constexpr (Op::NS > 0) TG_TRY((tg_launch_hub_merge<Op>(p, s, stream, name)));
+        return TG_OK;
+    };
+    st = launch_all();
+    for (int i = 0; i < 2; ++i) {
+        if (!forked[i]) continue;
+        if (cudaEventRecord(aux->join[i], aux->s[i]) != cudaSuccess || cudaStreamWaitEvent(stream, aux->join[i], 0) != cudaSuccess) {
+            if (st == TG_OK) { tg_set_error("%s: joining the auxiliary stream failed: %s", name, cudaGetErrorString(cudaGetLastError())); st = TG_ERR_CUDA; }
+        }
     }
-    if (n_big > 0) {
-        cudaStream_t st = fork ? aux->s[0] : stream;
-        if (fork) TG_CUDA(cudaStreamWaitEvent(st, aux->fork, 0));
-        const unsigned grid = (unsigned)((n_big + rows_per_cta - 1) / rows_per_cta);
-        tg_group_kernel<Op, Pol::U_PIPE, Pol::CTAS_PIPE, Pol::WARP_PIPE><<<grid, TG_GROUP_CTA_WARPS * 32, 0, st>>>(p, s.rows, n_big);
-        TG_LAUNCH_CHECK(name);
-        if (fork) TG_CUDA(cudaEventRecord(aux->join[0], st));
-    }
-    if (n_small > 0) {
-        cudaStream_t st = fork ? aux->s[1] : stream;
-        if (fork) TG_CUDA(cudaStreamWaitEvent(st, aux->fork, 0));
-        const unsigned grid = (unsigned)((n_small + rows_per_cta - 1) / rows_per_cta);
-        tg_group_kernel<Op, Pol::U_PLAIN, Pol::CTAS_PLAIN, false><<<grid, TG_GROUP_CTA_WARPS * 32, 0, st>>>(p, s.rows + n_big, n_small);
-        TG_LAUNCH_CHECK(name);
-        if (fork) TG_CUDA(cudaEventRecord(aux->join[1], st));
-    }
-    if constexpr (Op::NS > 0) TG_TRY((tg_launch_hub_merge<Op>(p, s, stream, name)));
-    if (fork) {
-        if (n_big > 0) TG_CUDA(cudaStreamWaitEvent(stream, aux->join[0], 0));
-        if (n_small > 0) TG_CUDA(cudaStreamWaitEvent(stream, aux->join[1], 0));
-    }
-    return TG_OK;
+    return st;
 }
