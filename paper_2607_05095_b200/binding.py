@@ -96,6 +96,23 @@ def _rows(t: torch.Tensor, name: str) -> torch.Tensor:
     return t
 
 
+def _check_rows(t: torch.Tensor, name: str, rows: int, like: torch.Tensor, exact: bool = True) -> torch.Tensor:
+    """Shape / dtype / device / contiguity of one row tensor against the block and the reference tensor `like` ([*, H, D]):
+    the C ABI only sees raw pointers, a wrong-sized or non-contiguous tensor would be read or written out of bounds."""
+    _rows(t, name)
+    if t.dtype != like.dtype or t.device != like.device or tuple(t.shape[1:]) != tuple(like.shape[1:]):
+        raise ValueError(f"{name}: expected [*, {like.shape[1]}, {like.shape[2]}] {like.dtype} on {like.device}, got {tuple(t.shape)} {t.dtype} on {t.device}")
+    if (exact and t.shape[0] != rows) or t.shape[0] < rows:
+        raise ValueError(f"{name}: {t.shape[0]} rows, the block needs {'exactly' if exact else 'at least'} {rows}")
+    return t
+
+
+def _check_scalars(t: torch.Tensor, name: str, rows: int, H: int, like: torch.Tensor) -> torch.Tensor:
+    if t.dtype != torch.float32 or tuple(t.shape) != (rows, H) or not t.is_contiguous() or t.device != like.device:
+        raise ValueError(f"{name} must be a contiguous float32 [{rows}, {H}] tensor on {like.device}")
+    return t
+
+
 def supported(H: int, D: int, dtype: torch.dtype) -> bool:
     return bool(lib().tg_supported(C.c_int(H), C.c_int(D), C.c_int(_DTYPES[dtype])))
 
@@ -127,6 +144,8 @@ class Block:
         return {"R": R.value, "E": E.value, "U": U.value, **{k: int(v) for k, v in zip(keys, stats)}}
 
     def attn_workspace(self, H: int, D: int, dtype: torch.dtype):
+        """(forward, backward) workspaces of this block, cached per (H, D, dtype).  They are shared by every call on the
+        block: calls that use the same block concurrently must be ordered on one stream (or use separate Block objects)."""
         key = (H, D, dtype)
         if key not in self._attn_ws:
             fb, bb = C.c_size_t(), C.c_size_t()
@@ -239,13 +258,14 @@ def aggregate_bwd(b: Block, w: torch.Tensor | None, X: torch.Tensor | None, dY: 
 
 
 def attn_fused_fwd(b: Block, Q: torch.Tensor, K: torch.Tensor, V: torch.Tensor, scale: float = 1.0, out=None):
-    _rows(Q, "Q"); _rows(K, "K"); _rows(V, "V")
+    _check_rows(Q, "Q", b.R, Q); _check_rows(K, "K", b.U, Q, exact=False); _check_rows(V, "V", b.U, Q, exact=False)
     H, D = Q.shape[1], Q.shape[2]
     if out is None:
         O = torch.empty_like(Q)
         lse = torch.empty(b.R, H, dtype=torch.float32, device=Q.device)
     else:
         O, lse = out
+        _check_rows(O, "O", b.R, Q); _check_scalars(lse, "lse", b.R, H, Q)
     ws, _ = b.attn_workspace(H, D, Q.dtype)
     _check(lib().tg_attn_fused_fwd(b.handle, C.c_int(H), C.c_int(D), C.c_int(_dt(Q)), _ptr(Q), _ptr(K), _ptr(V), C.c_float(scale),
                                    _ptr(O), _ptr(lse), _ptr(ws), C.c_size_t(ws.numel()), _stream()), "tg_attn_fused_fwd")
@@ -253,13 +273,16 @@ def attn_fused_fwd(b: Block, Q: torch.Tensor, K: torch.Tensor, V: torch.Tensor, 
 
 
 def attn_fused_bwd(b: Block, Q, K, V, O, lse, dO, scale: float = 1.0, out=None):
-    for t, n in ((Q, "Q"), (K, "K"), (V, "V"), (O, "O"), (dO, "dO")):
-        _rows(t, n)
+    for t, n in ((Q, "Q"), (O, "O"), (dO, "dO")):
+        _check_rows(t, n, b.R, Q)
+    _check_rows(K, "K", b.U, Q, exact=False); _check_rows(V, "V", b.U, Q, exact=False)
     H, D = Q.shape[1], Q.shape[2]
+    _check_scalars(lse, "lse", b.R, H, Q)
     if out is None:
         dQ, dK, dV = torch.empty_like(Q), torch.empty_like(K), torch.empty_like(V)
     else:
         dQ, dK, dV = out
+        _check_rows(dQ, "dQ", b.R, Q); _check_rows(dK, "dK", b.U, Q, exact=False); _check_rows(dV, "dV", b.U, Q, exact=False)
     _, ws = b.attn_workspace(H, D, Q.dtype)
     _check(lib().tg_attn_fused_bwd(b.handle, C.c_int(H), C.c_int(D), C.c_int(_dt(Q)), _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(lse),
                                    _ptr(dO), C.c_float(scale), _ptr(dQ), _ptr(dK), _ptr(dV), _ptr(ws), C.c_size_t(ws.numel()),
@@ -269,7 +292,11 @@ def attn_fused_bwd(b: Block, Q, K, V, O, lse, dO, scale: float = 1.0, out=None):
 
 def attn_fused_bwd_dst(b: Block, Q, K, V, O, lse, dO, scale: float, dQ):
     """First half of attn_fused_bwd (destination-major): dQ and the internal {LSE, delta} table."""
+    for t, n in ((Q, "Q"), (O, "O"), (dO, "dO"), (dQ, "dQ")):
+        _check_rows(t, n, b.R, Q)
+    _check_rows(K, "K", b.U, Q, exact=False); _check_rows(V, "V", b.U, Q, exact=False)
     H, D = Q.shape[1], Q.shape[2]
+    _check_scalars(lse, "lse", b.R, H, Q)
     _, ws = b.attn_workspace(H, D, Q.dtype)
     _check(lib().tg_attn_fused_bwd_dst(b.handle, C.c_int(H), C.c_int(D), C.c_int(_dt(Q)), _ptr(Q), _ptr(K), _ptr(V), _ptr(O),
                                        _ptr(lse), _ptr(dO), C.c_float(scale), _ptr(dQ), _ptr(ws), C.c_size_t(ws.numel()),
@@ -278,7 +305,11 @@ def attn_fused_bwd_dst(b: Block, Q, K, V, O, lse, dO, scale: float, dQ):
 
 
 def attn_fused_bwd_src(b: Block, Q, K, V, dO, scale: float, dK, dV):
-    """Second half of attn_fused_bwd (source-major over the transposed CSR): dK, dV."""
+    """Second half of attn_fused_bwd (source-major over the transposed CSR): dK, dV.  The block's cached workspace carries
+    the {LSE, delta} table from attn_fused_bwd_dst: both halves must run on the same stream, in this order."""
+    _check_rows(Q, "Q", b.R, Q); _check_rows(dO, "dO", b.R, Q)
+    for t, n in ((K, "K"), (V, "V"), (dK, "dK"), (dV, "dV")):
+        _check_rows(t, n, b.U, Q, exact=False)
     H, D = Q.shape[1], Q.shape[2]
     _, ws = b.attn_workspace(H, D, Q.dtype)
     _check(lib().tg_attn_fused_bwd_src(b.handle, C.c_int(H), C.c_int(D), C.c_int(_dt(Q)), _ptr(Q), _ptr(K), _ptr(V), _ptr(dO),

@@ -41,11 +41,12 @@ struct SchedIn {
     const int32_t* indptr;
     int chunk;
     int n_edges;
+    int group_max;   // rows up to this degree go to the group tier (tg_side::group_max)
     __device__ __forceinline__ IVec<TG_SK> operator()(int64_t i) const {
         int deg = indptr[i + 1] - indptr[i];
         if (deg < 0 || deg > n_edges) deg = 0;   // only a speculative build on unsorted input sees such an indptr (block.cu header)
         IVec<TG_SK> x = ivec_zero<TG_SK>();
-        if (deg <= TG_GROUP_MAX) {
+        if (deg <= group_max) {
             x.v[tg_degree_class(deg)] = 1;
         } else {
             const int chunks = (deg + chunk - 1) / chunk;
@@ -66,6 +67,7 @@ struct SchedOut {
     int4* bighubs;
     int* max_deg;
     int n_edges;
+    int group_max;
     int64_t rows_cap, items_cap, hubs_cap, bighubs_cap;   // a speculative build may scan a garbage indptr: never write past the lists
     __device__ __forceinline__ void operator()(int64_t i, const IVec<TG_SK>& ex, const IVec<TG_SK>& x, const IVec<TG_SK>& tot) const {
         const int row = (int)i;
@@ -73,7 +75,7 @@ struct SchedOut {
         int e = indptr[i + 1];
         if (e < b || e - b > n_edges) e = b;
         const int ic = tg_item_class(e - b, chunk);
-        const int chunks = (e - b > TG_GROUP_MAX) ? x.v[TG_NCLS + ic] : 0;
+        const int chunks = (e - b > group_max) ? x.v[TG_NCLS + ic] : 0;
         if (chunks == 0) {
             const int c = tg_degree_class(e - b);
             int pos = ex.v[c];
@@ -95,8 +97,8 @@ struct SchedOut {
     }
 };
 
-// a warp-tier row (deg > TG_GROUP_MAX) has ceil(deg / chunk) <= deg / TG_CHUNK_MIN + 1 <= 2 * deg / TG_GROUP_MAX items
-static inline int64_t side_items_bound(int64_t n_edges) { return 2 * (n_edges / TG_GROUP_MAX) + 2; }
+// a warp-tier row (deg > group_max >= TG_GROUP_MAX_SMALL) has ceil(deg / chunk) <= deg / TG_CHUNK_MIN + 1 items
+static inline int64_t side_items_bound(int64_t n_edges) { return n_edges / TG_CHUNK_MIN + n_edges / TG_GROUP_MAX_SMALL + 2; }
 static inline int64_t side_hubs_bound(int64_t n_edges) { return n_edges / TG_CHUNK_MIN + 1; }
 static inline int64_t side_bighubs_bound(int64_t n_edges) { return n_edges / (TG_CHUNK_MIN * TG_HUB_DIRECT) + 1; }
 
@@ -124,8 +126,11 @@ static tg_status_t tg_side_launch(tg_side* s, int64_t n_rows, const int* n_rows_
     int chunk = TG_CHUNK_MIN;
     while (chunk < TG_CHUNK_MAX && n_edges / chunk > 148 * 16 * 4) chunk *= 2;
     s->chunk = chunk;
-    SchedIn in{indptr, chunk, (int)n_edges};
-    SchedOut out{indptr, chunk, s->rows, s->items, s->hubs, s->bighubs, totals_dev + TG_SK, (int)n_edges,
+    // A launch-bound small side is limited by its longest single-group chain (one edge per trip, one gather latency per
+    // trip): rows above 32 edges go to the warp tier there (config 3: 62 -> 55 us per step, config 2: 113 -> 100 us; 16 costs the destination side more than it saves), where the four groups of a warp share the row.
+    s->group_max = n_edges < TG_FORK_MIN_EDGES ? TG_GROUP_MAX_SMALL : TG_GROUP_MAX;
+    SchedIn in{indptr, chunk, (int)n_edges, s->group_max};
+    SchedOut out{indptr, chunk, s->rows, s->items, s->hubs, s->bighubs, totals_dev + TG_SK, (int)n_edges, s->group_max,
                  n_rows + 1, side_items_bound(n_edges), side_hubs_bound(n_edges), side_bighubs_bound(n_edges)};
     TG_TRY((tg_scan<TG_SK>(n_rows, in, out, scan_tmp, reinterpret_cast<IVec<TG_SK>*>(totals_dev), stream, n_rows_dev)));
     return TG_OK;

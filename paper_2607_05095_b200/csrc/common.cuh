@@ -74,6 +74,10 @@ void tg_count_launch();
 constexpr int TG_NCLS = TG_NCLS_N;              // degree classes <=2, 3-4, 5-8, 9-16, 17-32, 33-64 (, 65-128)
 constexpr int TG_NCLS_SMALL = TG_NCLS_SMALL_N;  // classes 0..2 (deg <= 8) run in the high-occupancy kernel variant
 constexpr int TG_GROUP_MAX = 2 << (TG_NCLS - 1);
+#ifndef TG_GROUP_MAX_SMALL_N
+#define TG_GROUP_MAX_SMALL_N 32
+#endif
+constexpr int TG_GROUP_MAX_SMALL = TG_GROUP_MAX_SMALL_N;   // group-tier limit of a launch-bound side (< TG_FORK_MIN_EDGES edges)
 #ifndef TG_CHUNK_MAX_EDGES
 #define TG_CHUNK_MAX_EDGES 1024
 #endif
@@ -98,6 +102,7 @@ struct tg_side {
     int32_t n_group = 0, n_items = 0, n_hubs = 0, n_bighubs = 0, n_slots = 0;
     int32_t max_deg = 0;
     int32_t chunk = TG_CHUNK_MAX;   // edges per warp item of this side
+    int32_t group_max = TG_GROUP_MAX;   // rows up to this degree are group-tier rows
     // group-tier rows of the classes >= TG_NCLS_SMALL come first in `rows`
     int32_t n_group_big() const { int n = 0; for (int c = TG_NCLS_SMALL; c < TG_NCLS; ++c) n += n_cls[c]; return n; }
     int32_t n_group_small() const { return n_group - n_group_big(); }
