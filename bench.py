@@ -485,6 +485,9 @@ def run_ours(args):
         d = {n: hostbuf[n].cuda() for n in ("q", "k", "v", "do")}
         out = dict(O=torch.empty_like(d["q"]), lse=torch.empty(w.R, w.H, dtype=torch.float32, device="cuda"),
                    dQ=torch.empty_like(d["q"]), dK=torch.empty_like(d["k"]), dV=torch.empty_like(d["v"]))
+        # --side-copy (bf16 storage): the forward also writes a float32 copy of O and the backward takes delta from it
+        # (DESIGN.md §6.2).  Measured on config 4: fwd +0.024 ms, bwd_dst -0.020 ms: no gain, so it is off by default.
+        out["o32"] = torch.empty(w.R, w.H, w.D, dtype=torch.float32, device="cuda") if (w.dtype == "bf16" and args.side_copy) else None
         blocks.append(dict(w=w, blk=blk, host=hostbuf, dev=d, out=out, info=blk.info()))
     cfg, comp = config_dict(args, ws, [b["blk"].U for b in blocks])
     small = comp <= 2.5e8                                      # configs 1-3: working set fits in L2, launch-bound
@@ -494,9 +497,9 @@ def run_ours(args):
         for bi, b in enumerate(blocks):
             w, blk, d, o = b["w"], b["blk"], b["dev"], b["out"]
             if ev is not None: ev[bi][0].record()
-            B.attn_fused_fwd(blk, d["q"], d["k"], d["v"], w.scale, out=(o["O"], o["lse"]))
+            B.attn_fused_fwd(blk, d["q"], d["k"], d["v"], w.scale, out=(o["O"], o["lse"]), o32=o["o32"])
             if ev is not None: ev[bi][1].record()
-            B.attn_fused_bwd_dst(blk, d["q"], d["k"], d["v"], o["O"], o["lse"], d["do"], w.scale, o["dQ"])
+            B.attn_fused_bwd_dst(blk, d["q"], d["k"], d["v"], o["O"], o["lse"], d["do"], w.scale, o["dQ"], o32=o["o32"])
             if ev is not None: ev[bi][2].record()
             B.attn_fused_bwd_src(blk, d["q"], d["k"], d["v"], d["do"], w.scale, o["dK"], o["dV"])
             if ev is not None: ev[bi][3].record()
@@ -600,7 +603,10 @@ def run_ours(args):
     comp_all = comp * (E_all / max(E_local, 1))               # every rank runs a block of the same recipe
     hbm_gbs = comp_all / (ms_per_step * 1e-3) / 1e9
     hbm = {"compulsory_bytes_per_step": comp, "achieved_gbs": hbm_gbs, "frac_of_8TBs": hbm_gbs / HBM_NOMINAL_GBS / world,
-           "frac_of_measured_copy": hbm_gbs / peak / world, "sum_of_call_bytes": sum(sum(call_bytes(x["w"].R, x["w"].E, x["blk"].U, x["w"].H, x["w"].D,
+           "frac_of_measured_copy": hbm_gbs / peak / world,
+           "fp32_side_copy_of_O": {"used": any(x["out"]["o32"] is not None for x in blocks),
+                                   "extra_bytes_per_step_not_counted": sum(2 * x["out"]["o32"].numel() * 4 for x in blocks if x["out"]["o32"] is not None)},
+           "sum_of_call_bytes": sum(sum(call_bytes(x["w"].R, x["w"].E, x["blk"].U, x["w"].H, x["w"].D,
                                                                                         2 if x["w"].dtype == "bf16" else 4, x["w"].dedup_mode).values()) for x in blocks)}
 
     extras = {"launch": {"mode": launch_mode, "eager_ms_per_step": eager_ms / args.steps,
@@ -636,7 +642,8 @@ def run_ours(args):
     for bb in blocks:
         bb["hout"] = {n: torch.empty(bb["out"][n].shape, dtype=bb["out"][n].dtype).pin_memory() for n in OUT}
         bb["din"] = [{n: torch.empty_like(bb["host"][n], device="cuda") for n in IN} for _ in range(NB)]
-        bb["dout"] = [{n: torch.empty_like(bb["out"][n]) for n in OUT + ("lse",)} for _ in range(NB)]
+        bb["dout"] = [{**{n: torch.empty_like(bb["out"][n]) for n in OUT + ("lse",)},
+                       "o32": None if bb["out"]["o32"] is None else torch.empty_like(bb["out"]["o32"])} for _ in range(NB)]
         h2d += sum(t.numel() * t.element_size() for t in bb["host"].values())
         d2h += sum(t.numel() * t.element_size() for t in bb["hout"].values())
 
@@ -655,8 +662,8 @@ def run_ours(args):
             for bb in blocks:
                 ww, di, do_ = bb["w"], bb["din"][k], bb["dout"][k]
                 blk = B.block_build(ww.R, di["root"], di["nbr"], None, None, ww.dedup_mode)
-                O, lse = B.attn_fused_fwd(blk, di["q"], di["k"], di["v"], ww.scale, out=(do_["O"], do_["lse"]))
-                B.attn_fused_bwd(blk, di["q"], di["k"], di["v"], O, lse, di["do"], ww.scale, out=(do_["dQ"], do_["dK"], do_["dV"]))
+                O, lse = B.attn_fused_fwd(blk, di["q"], di["k"], di["v"], ww.scale, out=(do_["O"], do_["lse"]), o32=do_["o32"])
+                B.attn_fused_bwd(blk, di["q"], di["k"], di["v"], O, lse, di["do"], ww.scale, out=(do_["dQ"], do_["dK"], do_["dV"]), o32=do_["o32"])
             ev_cmp[k].record(s_cmp)
 
     def e2e_d2h(k):
@@ -730,6 +737,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-unfused", action="store_true", help="skip the extras: unfused chain, edge term, SlimCache, plain AGG, sampler")
     ap.add_argument("--no-sampler", action="store_true")
+    ap.add_argument("--side-copy", action="store_true", help="bf16 storage: the forward writes a float32 side copy of O, the backward takes delta from it")
     args = ap.parse_args()
     if args.probe_gather:
         from paper_2607_05095_b200 import binding as B

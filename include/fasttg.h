@@ -227,20 +227,24 @@ TG_API tg_status_t tg_attn_workspace_bytes(const tg_block_t* b, int H, int D, tg
                                            size_t* fwd_bytes /*HOST*/, size_t* bwd_bytes /*HOST*/);
 
 /* Forward:  s = scale*<Q[v(e)],K[r(e)]>, alpha = softmax over N(v), O[v] = sum alpha*V[r(e)],
- *           LSE[v,h] = m + ln l (natural log).  Q,O [R,H,D]; K,V [U,H,D]; LSE [R,H] float32. */
+ *           LSE[v,h] = m + ln l (natural log).  Q,O [R,H,D]; K,V [U,H,D]; LSE [R,H] float32.
+ * o_f32 (nullable, [R,H,D] float32, 16-byte aligned): an unrounded copy of O for the backward.  Meant for TG_BF16
+ *           storage, where it lets the backward take delta = <dO, O> up front instead of accumulating it from the
+ *           edges; R*H*D*4 extra bytes written here and read there, not part of the compulsory bytes. */
 TG_API tg_status_t tg_attn_fused_fwd(const tg_block_t* b, int H, int D, tg_dtype_t dtype,
                                      const void* Q, const void* K, const void* V, float scale,
-                                     void* O, float* lse, void* ws, size_t ws_bytes, tg_stream_t stream);
+                                     void* O, float* lse, float* o_f32, void* ws, size_t ws_bytes, tg_stream_t stream);
 
 /* Backward for upstream gradient dO:
  *   delta[v,h] = <dO[v,h,:], O[v,h,:]>;  alpha = exp(s - LSE);  dalpha = <dO[v(e)], V[r(e)]>;
  *   ds = alpha*(dalpha - delta);  dQ[v] = scale * sum_{N(v)} ds*K[r(e)];
  *   dK[u] = scale * sum_{r(e)=u} ds*Q[v(e)];  dV[u] = sum_{r(e)=u} alpha*dO[v(e)].
  * O and lse are the forward's outputs.  dQ [R,H,D]; dK,dV [U,H,D].
- * (With TG_BF16 storage delta is accumulated as sum alpha*dalpha in fp32 and O is only validated, not read:
- *  the bf16 rounding of O would otherwise leak into dQ.) */
+ * TG_BF16 storage: the bf16 rounding of O would leak into dQ through delta, so delta comes either from
+ * o_f32 (the forward's float32 copy of O, if given) or, with o_f32 == NULL, from the edges (sum alpha*dalpha in fp32,
+ * one more accumulator per lane); O itself is then only validated, not read.  TG_F32 storage ignores o_f32. */
 TG_API tg_status_t tg_attn_fused_bwd(const tg_block_t* b, int H, int D, tg_dtype_t dtype,
-                                     const void* Q, const void* K, const void* V, const void* O,
+                                     const void* Q, const void* K, const void* V, const void* O, const float* o_f32,
                                      const float* lse, const void* dO, float scale,
                                      void* dQ, void* dK, void* dV,
                                      void* ws, size_t ws_bytes, tg_stream_t stream);
@@ -255,7 +259,7 @@ TG_API tg_status_t tg_attn_fused_bwd(const tg_block_t* b, int H, int D, tg_dtype
  * {LSE, delta} table into `ws`; _src: source-major over the transposed CSR, reads that table from the
  * SAME `ws`, writes dK and dV.  Arguments as in tg_attn_fused_bwd. */
 TG_API tg_status_t tg_attn_fused_bwd_dst(const tg_block_t* b, int H, int D, tg_dtype_t dtype,
-                                         const void* Q, const void* K, const void* V, const void* O,
+                                         const void* Q, const void* K, const void* V, const void* O, const float* o_f32,
                                          const float* lse, const void* dO, float scale, void* dQ,
                                          void* ws, size_t ws_bytes, tg_stream_t stream);
 TG_API tg_status_t tg_attn_fused_bwd_src(const tg_block_t* b, int H, int D, tg_dtype_t dtype,

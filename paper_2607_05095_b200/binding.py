@@ -257,7 +257,14 @@ def aggregate_bwd(b: Block, w: torch.Tensor | None, X: torch.Tensor | None, dY: 
     return dX, dw
 
 
-def attn_fused_fwd(b: Block, Q: torch.Tensor, K: torch.Tensor, V: torch.Tensor, scale: float = 1.0, out=None):
+def _check_o32(o32, b: Block, Q: torch.Tensor):
+    if o32 is not None and (o32.dtype != torch.float32 or tuple(o32.shape) != (b.R,) + tuple(Q.shape[1:]) or not o32.is_contiguous() or o32.device != Q.device):
+        raise ValueError(f"o32 must be a contiguous float32 [{b.R}, {Q.shape[1]}, {Q.shape[2]}] tensor on {Q.device}")
+    return o32
+
+
+def attn_fused_fwd(b: Block, Q: torch.Tensor, K: torch.Tensor, V: torch.Tensor, scale: float = 1.0, out=None, o32: torch.Tensor | None = None):
+    """tg_attn_fused_fwd.  o32 (optional, float32 [R,H,D]): receives the unrounded copy of O for attn_fused_bwd (bf16 storage)."""
     _check_rows(Q, "Q", b.R, Q); _check_rows(K, "K", b.U, Q, exact=False); _check_rows(V, "V", b.U, Q, exact=False)
     H, D = Q.shape[1], Q.shape[2]
     if out is None:
@@ -268,11 +275,11 @@ def attn_fused_fwd(b: Block, Q: torch.Tensor, K: torch.Tensor, V: torch.Tensor, 
         _check_rows(O, "O", b.R, Q); _check_scalars(lse, "lse", b.R, H, Q)
     ws, _ = b.attn_workspace(H, D, Q.dtype)
     _check(lib().tg_attn_fused_fwd(b.handle, C.c_int(H), C.c_int(D), C.c_int(_dt(Q)), _ptr(Q), _ptr(K), _ptr(V), C.c_float(scale),
-                                   _ptr(O), _ptr(lse), _ptr(ws), C.c_size_t(ws.numel()), _stream()), "tg_attn_fused_fwd")
+                                   _ptr(O), _ptr(lse), _ptr(_check_o32(o32, b, Q)), _ptr(ws), C.c_size_t(ws.numel()), _stream()), "tg_attn_fused_fwd")
     return O, lse
 
 
-def attn_fused_bwd(b: Block, Q, K, V, O, lse, dO, scale: float = 1.0, out=None):
+def attn_fused_bwd(b: Block, Q, K, V, O, lse, dO, scale: float = 1.0, out=None, o32=None):
     for t, n in ((Q, "Q"), (O, "O"), (dO, "dO")):
         _check_rows(t, n, b.R, Q)
     _check_rows(K, "K", b.U, Q, exact=False); _check_rows(V, "V", b.U, Q, exact=False)
@@ -284,13 +291,13 @@ def attn_fused_bwd(b: Block, Q, K, V, O, lse, dO, scale: float = 1.0, out=None):
         dQ, dK, dV = out
         _check_rows(dQ, "dQ", b.R, Q); _check_rows(dK, "dK", b.U, Q, exact=False); _check_rows(dV, "dV", b.U, Q, exact=False)
     _, ws = b.attn_workspace(H, D, Q.dtype)
-    _check(lib().tg_attn_fused_bwd(b.handle, C.c_int(H), C.c_int(D), C.c_int(_dt(Q)), _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(lse),
+    _check(lib().tg_attn_fused_bwd(b.handle, C.c_int(H), C.c_int(D), C.c_int(_dt(Q)), _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(_check_o32(o32, b, Q)), _ptr(lse),
                                    _ptr(dO), C.c_float(scale), _ptr(dQ), _ptr(dK), _ptr(dV), _ptr(ws), C.c_size_t(ws.numel()),
                                    _stream()), "tg_attn_fused_bwd")
     return dQ, dK, dV
 
 
-def attn_fused_bwd_dst(b: Block, Q, K, V, O, lse, dO, scale: float, dQ):
+def attn_fused_bwd_dst(b: Block, Q, K, V, O, lse, dO, scale: float, dQ, o32=None):
     """First half of attn_fused_bwd (destination-major): dQ and the internal {LSE, delta} table."""
     for t, n in ((Q, "Q"), (O, "O"), (dO, "dO"), (dQ, "dQ")):
         _check_rows(t, n, b.R, Q)
@@ -299,7 +306,7 @@ def attn_fused_bwd_dst(b: Block, Q, K, V, O, lse, dO, scale: float, dQ):
     _check_scalars(lse, "lse", b.R, H, Q)
     _, ws = b.attn_workspace(H, D, Q.dtype)
     _check(lib().tg_attn_fused_bwd_dst(b.handle, C.c_int(H), C.c_int(D), C.c_int(_dt(Q)), _ptr(Q), _ptr(K), _ptr(V), _ptr(O),
-                                       _ptr(lse), _ptr(dO), C.c_float(scale), _ptr(dQ), _ptr(ws), C.c_size_t(ws.numel()),
+                                       _ptr(_check_o32(o32, b, Q)), _ptr(lse), _ptr(dO), C.c_float(scale), _ptr(dQ), _ptr(ws), C.c_size_t(ws.numel()),
                                        _stream()), "tg_attn_fused_bwd_dst")
     return dQ
 

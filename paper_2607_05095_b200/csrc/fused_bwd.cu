@@ -59,6 +59,8 @@
 #define TG_BWD2_MMA 0
 #endif
 
+template <class X> struct tg_type_tag { using type = X; };
+
 struct BwdArgs {
     const tg_block* b;
     const void *Q, *K, *V, *O, *dO;
@@ -69,6 +71,7 @@ struct BwdArgs {
     size_t ws_bytes;
     int H;
     cudaStream_t stream;
+    const float* O32;
 };
 
 template <class Tr>
@@ -87,20 +90,27 @@ struct BwdFn {
             // wide fp32 rows: 16 words per lane (LPR 8) and a single gather buffer, as in the source-major pass below
             constexpr bool WIDE1 = !Tr::BF16 && Tr::F * Tr::EB >= 512;
             using Tr1 = RowTraits<T, Tr::H, Tr::D, WIDE1 ? 16 : 8>;
-            using Op = Bwd1Op<Tr1>;
-            static_assert(Tr1::NE * Tr1::LPR <= Tr::NE * Tr::LPR, "the partial workspace is sized with the default layout");
-            typename Op::Params p;
-            p.Q = static_cast<const T*>(a.Q); p.K = static_cast<const T*>(a.K); p.V = static_cast<const T*>(a.V);
-            p.O = static_cast<const T*>(a.O); p.dO = static_cast<const T*>(a.dO);
-            p.kv = a.b->kv_row; p.lse = a.lse;
-            p.dQ = static_cast<T*>(a.dQ); p.ld = ld; p.part = dq_part;
-            p.scale = a.scale; p.scale2 = a.scale * TG_LOG2E;
-            if constexpr (WIDE1)
-                TG_TRY((tg_launch_tiers<Op, TierPolicy<1, 2, 1, 2, 1, 16, false>>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst")));
-            else {
-                using OpW = typename tg_warp_op<Op, (TG_BWD1_MMA != 0) && MmaDotOk<Tr1>::value>::type;
-                TG_TRY((tg_launch_tiers<Op, TierPolicy<TG_BWD1_POLICY>, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst")));
-            }
+            auto launch = [&](auto tag) -> tg_status_t {
+                using Op = typename decltype(tag)::type;
+                static_assert(Tr1::NE * Tr1::LPR <= Tr::NE * Tr::LPR, "the partial workspace is sized with the default layout");
+                typename Op::Params p;
+                p.Q = static_cast<const T*>(a.Q); p.K = static_cast<const T*>(a.K); p.V = static_cast<const T*>(a.V);
+                p.O = static_cast<const T*>(a.O); p.dO = static_cast<const T*>(a.dO);
+                p.kv = a.b->kv_row; p.lse = a.lse;
+                p.dQ = static_cast<T*>(a.dQ); p.ld = ld; p.part = dq_part;
+                p.scale = a.scale; p.scale2 = a.scale * TG_LOG2E;
+                p.O32 = a.O32;
+                if constexpr (WIDE1) {
+                    return tg_launch_tiers<Op, TierPolicy<1, 2, 1, 2, 1, 16, false>>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst");
+                } else {
+                    using OpW = typename tg_warp_op<Op, (TG_BWD1_MMA != 0) && MmaDotOk<Tr1>::value>::type;
+                    return tg_launch_tiers<Op, TierPolicy<TG_BWD1_POLICY>, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst");
+                }
+            };
+            // bf16 storage: with the forward's fp32 copy of O delta = <dO, O> is taken up front (one accumulator and 16 registers
+            // fewer per lane); without it delta is accumulated from the edges
+            if (Tr::BF16 && a.O32) TG_TRY(launch(tg_type_tag<Bwd1Op<Tr1, false>>{}));
+            else TG_TRY(launch(tg_type_tag<Bwd1Op<Tr1>>{}));
         }
         if (which & 2) {
             // wide fp32 rows: 16 words per lane (LPR 8) and a single gather buffer; the lane layout is private to a kernel
@@ -126,7 +136,7 @@ struct BwdFn {
 };
 
 static tg_status_t bwd_common(const tg_block_t* b, int H, int D, tg_dtype_t dtype, const void* Q, const void* K, const void* V,
-                              const void* O, const float* lse, const void* dO, float scale, void* dQ, void* dK, void* dV,
+                              const void* O, const float* o_f32, const float* lse, const void* dO, float scale, void* dQ, void* dK, void* dV,
                               void* ws, size_t ws_bytes, tg_stream_t stream, int which) {
     TG_CHECK_PTR(b);
     if (!tg_shape_supported(H, D, dtype)) TG_FAIL(TG_ERR_UNSUPPORTED, "unsupported (H=%d, D=%d, dtype=%d)", H, D, (int)dtype);
@@ -138,24 +148,25 @@ static tg_status_t bwd_common(const tg_block_t* b, int H, int D, tg_dtype_t dtyp
         if (which & 2) { TG_CHECK_ROWS(dK); TG_CHECK_ROWS(dV); }
     }
     if (!ws) TG_FAIL(TG_ERR_WORKSPACE, "fused bwd needs a workspace (tg_attn_workspace_bytes)");
-    BwdArgs a{b, Q, K, V, O, dO, lse, scale, dQ, dK, dV, ws, ws_bytes, H, static_cast<cudaStream_t>(stream)};
+    if (o_f32 && (reinterpret_cast<uintptr_t>(o_f32) & 15u)) TG_FAIL(TG_ERR_ALIGNMENT, "o_f32 is not 16-byte aligned");
+    BwdArgs a{b, Q, K, V, O, dO, lse, scale, dQ, dK, dV, ws, ws_bytes, H, static_cast<cudaStream_t>(stream), o_f32};
     return tg_dispatch<BwdFn>(H, D, dtype, a, which);
 }
 
 extern "C" tg_status_t tg_attn_fused_bwd(const tg_block_t* b, int H, int D, tg_dtype_t dtype, const void* Q, const void* K,
-                                         const void* V, const void* O, const float* lse, const void* dO, float scale,
+                                         const void* V, const void* O, const float* o_f32, const float* lse, const void* dO, float scale,
                                          void* dQ, void* dK, void* dV, void* ws, size_t ws_bytes, tg_stream_t stream) {
-    return bwd_common(b, H, D, dtype, Q, K, V, O, lse, dO, scale, dQ, dK, dV, ws, ws_bytes, stream, 3);
+    return bwd_common(b, H, D, dtype, Q, K, V, O, o_f32, lse, dO, scale, dQ, dK, dV, ws, ws_bytes, stream, 3);
 }
 
 extern "C" tg_status_t tg_attn_fused_bwd_dst(const tg_block_t* b, int H, int D, tg_dtype_t dtype, const void* Q, const void* K,
-                                             const void* V, const void* O, const float* lse, const void* dO, float scale,
+                                             const void* V, const void* O, const float* o_f32, const float* lse, const void* dO, float scale,
                                              void* dQ, void* ws, size_t ws_bytes, tg_stream_t stream) {
-    return bwd_common(b, H, D, dtype, Q, K, V, O, lse, dO, scale, dQ, nullptr, nullptr, ws, ws_bytes, stream, 1);
+    return bwd_common(b, H, D, dtype, Q, K, V, O, o_f32, lse, dO, scale, dQ, nullptr, nullptr, ws, ws_bytes, stream, 1);
 }
 
 extern "C" tg_status_t tg_attn_fused_bwd_src(const tg_block_t* b, int H, int D, tg_dtype_t dtype, const void* Q, const void* K,
                                              const void* V, const void* dO, float scale, void* dK, void* dV, void* ws,
                                              size_t ws_bytes, tg_stream_t stream) {
-    return bwd_common(b, H, D, dtype, Q, K, V, nullptr, nullptr, dO, scale, nullptr, dK, dV, ws, ws_bytes, stream, 2);
+    return bwd_common(b, H, D, dtype, Q, K, V, nullptr, nullptr, nullptr, dO, scale, nullptr, dK, dV, ws, ws_bytes, stream, 2);
 }

@@ -41,6 +41,7 @@ struct FwdArgs {
     float* lse;
     void* ws;
     cudaStream_t stream;
+    float* O32;
 };
 
 template <class Tr>
@@ -56,6 +57,7 @@ struct FwdFn {
         p.lse = a.lse;
         p.part = static_cast<float*>(a.ws);
         p.scale2 = a.scale * TG_LOG2E;
+        p.O32 = a.O32;
         return tg_launch_tiers<Op, TierPolicy<TG_FWD_POLICY>, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_fwd");
     }
 };
@@ -73,7 +75,7 @@ extern "C" tg_status_t tg_attn_workspace_bytes(const tg_block_t* b, int H, int D
 }
 
 extern "C" tg_status_t tg_attn_fused_fwd(const tg_block_t* b, int H, int D, tg_dtype_t dtype, const void* Q, const void* K,
-                                         const void* V, float scale, void* O, float* lse, void* ws, size_t ws_bytes,
+                                         const void* V, float scale, void* O, float* lse, float* o_f32, void* ws, size_t ws_bytes,
                                          tg_stream_t stream) {
     TG_CHECK_PTR(b);
     if (!tg_shape_supported(H, D, dtype)) TG_FAIL(TG_ERR_UNSUPPORTED, "unsupported (H=%d, D=%d, dtype=%d)", H, D, (int)dtype);
@@ -84,6 +86,7 @@ extern "C" tg_status_t tg_attn_fused_fwd(const tg_block_t* b, int H, int D, tg_d
     TG_TRY(tg_get_geom(H, D, dtype, &g));
     const tg_attn_ws_sizes s = tg_attn_ws(b, H, g);
     if (s.fwd_part > 0 && (!ws || ws_bytes < s.fwd_part)) TG_FAIL(TG_ERR_WORKSPACE, "fused fwd needs %zu workspace bytes", s.fwd_part);
-    FwdArgs a{b, Q, K, V, scale, O, lse, ws, static_cast<cudaStream_t>(stream)};
+    if (o_f32 && (reinterpret_cast<uintptr_t>(o_f32) & 15u)) TG_FAIL(TG_ERR_ALIGNMENT, "o_f32 is not 16-byte aligned");
+    FwdArgs a{b, Q, K, V, scale, O, lse, ws, static_cast<cudaStream_t>(stream), o_f32};
     return tg_dispatch<FwdFn>(H, D, dtype, a);
 }

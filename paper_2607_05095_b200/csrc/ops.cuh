@@ -32,6 +32,7 @@ struct FwdOp {
         float* lse;
         float* part;
         float scale2;  // scale * log2(e)
+        float* O32;    // nullable: fp32 copy of O for the backward (bf16 storage: delta = <dO, O> without O's bf16 rounding)
     };
     struct Buf { RowReg<Tr> k, v; };
     const Params& p;
@@ -111,6 +112,7 @@ struct FwdOp {
         for (int j = 0; j < NHL; ++j) inv[j] = st[NHL + j] > 0.f ? 1.f / st[NHL + j] : 0.f;
         row_scale_heads(st + 2 * NHL, inv, lp);
         row_store(p.O + (size_t)row * Tr::F, lp, st + 2 * NHL, 1.f);
+        if (p.O32) row_store_f32<Tr>(p.O32 + (size_t)row * Tr::F, lp, st + 2 * NHL);
         if (lp.head_writer()) {
 #pragma unroll
             for (int j = 0; j < NHL; ++j)
@@ -132,11 +134,12 @@ struct FwdOp {
 //     d = sum alpha*dalpha}, dQ = scale*(A1 - d*A2).  One extra axpy per edge, O is not read.
 // Also writes ld[v,h] = {lse2, delta} for the source-major pass.
 // -------------------------------------------------------------------------------------------------
-template <class Tr_>
+template <class Tr_, bool EDGE_DELTA_ = Tr_::BF16>
 struct Bwd1Op {
     using Tr = Tr_;
     using T = typename Tr::T;
-    static constexpr bool EDGE_DELTA = Tr::BF16;
+    // bf16 storage without an fp32 copy of O: delta from the edges.  EDGE_DELTA_ = false with bf16 storage needs Params::O32.
+    static constexpr bool EDGE_DELTA = EDGE_DELTA_;
     static constexpr int NHL = Tr::NHL;
     static constexpr int NS = EDGE_DELTA ? 2 * Tr::NE + NHL : Tr::NE, NS1 = NS;
     struct Params {
@@ -147,6 +150,7 @@ struct Bwd1Op {
         float2* ld;
         float* part;
         float scale, scale2;
+        const float* O32;   // nullable: the forward's fp32 copy of O (bf16 storage)
     };
     struct Buf { RowReg<Tr> k, v; };
     const Params& p;
@@ -164,7 +168,12 @@ struct Bwd1Op {
         cur = row;
         row_load(q, p.Q + lp.off + (size_t)row * Tr::F, lp);
         row_load(g, p.dO + lp.off + (size_t)row * Tr::F, lp);
-        if constexpr (!EDGE_DELTA) {
+        if constexpr (!EDGE_DELTA && Tr::BF16) {      // delta = <dO, O> with O taken from its fp32 side copy
+            float of[Tr::NE], gf[Tr::NE];
+            row_load_f32<Tr>(of, p.O32 + (size_t)row * Tr::F, lp);
+            row_to_float(g, gf);
+            row_dotf_heads<Tr>(gf, of, lp, delta);
+        } else if constexpr (!EDGE_DELTA) {
             RowReg<Tr> o;
             row_load(o, p.O + lp.off + (size_t)row * Tr::F, lp);
             row_dot_heads(g, o, lp, delta);

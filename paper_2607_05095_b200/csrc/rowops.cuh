@@ -298,3 +298,57 @@ __device__ __forceinline__ void row_store(typename Tr::T* row, const LanePos<Tr>
         else *reinterpret_cast<uint32_t*>(a) = w[0];
     }
 }
+
+// fp32 view of a row in the lane layout (a side copy kept in float whatever the storage dtype): lane's slot k covers the
+// VEC consecutive floats of vector lig + LPR*k.
+template <class Tr>
+__device__ __forceinline__ void row_store_f32(float* row, const LanePos<Tr>& lp, const float* x) {
+#pragma unroll
+    for (int k = 0; k < Tr::NK; ++k) {
+        if (!lp.slot_valid(k)) continue;
+        float* a = row + (lp.lig + Tr::LPR * k) * Tr::VEC;
+#pragma unroll
+        for (int e = 0; e < Tr::VEC; ++e) a[e] = x[k * Tr::VEC + e];
+    }
+}
+template <class Tr>
+__device__ __forceinline__ void row_load_f32(float (&x)[Tr::NE], const float* row, const LanePos<Tr>& lp) {
+#pragma unroll
+    for (int k = 0; k < Tr::NK; ++k) {
+        const float* a = row + (lp.lig + Tr::LPR * k) * Tr::VEC;
+#pragma unroll
+        for (int e = 0; e < Tr::VEC; ++e) x[k * Tr::VEC + e] = lp.slot_valid(k) ? a[e] : 0.f;
+    }
+}
+// s[j] = <a, b> restricted to head slot j for two rows already widened to float (same reduction as row_dot_heads)
+template <class Tr, int k>
+__device__ __forceinline__ void dotf_slots(const float* a, const float* b, const LanePos<Tr>& lp, float (&s)[Tr::NHL]) {
+    if constexpr (k < Tr::NK) {
+        float part = 0.f;
+#pragma unroll
+        for (int e = Tr::VEC * k; e < Tr::VEC * (k + 1); ++e) part = fmaf(a[e], b[e], part);
+        if constexpr (Tr::MODE_A) {
+            s[k] = part;
+        } else if constexpr (Tr::slot_lo(k) == Tr::slot_hi(k)) {
+            s[Tr::slot_lo(k)] += part;
+        } else {
+            const bool hi = (lp.mix >> k) & 1u;
+            s[Tr::slot_lo(k)] += hi ? 0.f : part;
+            s[Tr::slot_hi(k)] += hi ? part : 0.f;
+        }
+        dotf_slots<Tr, k + 1>(a, b, lp, s);
+    }
+}
+template <class Tr>
+__device__ __forceinline__ void row_dotf_heads(const float* a, const float* b, const LanePos<Tr>& lp, float (&s)[Tr::NHL]) {
+    if constexpr (!Tr::MODE_A) {
+#pragma unroll
+        for (int j = 0; j < Tr::NHL; ++j) s[j] = 0.f;
+    }
+    dotf_slots<Tr, 0>(a, b, lp, s);
+#pragma unroll
+    for (int o = 1; o < Tr::S; o <<= 1) {
+#pragma unroll
+        for (int j = 0; j < Tr::NHL; ++j) s[j] += __shfl_xor_sync(0xffffffffu, s[j], o);
+    }
+}

@@ -60,11 +60,13 @@ def assert_close(name, got, ref, dtype, extra_atol=0.0):
     return used
 
 
-def run_fused(B, blk, w, feats, scale):
-    """GPU fused forward + backward through the C ABI; returns host float arrays."""
+def run_fused(B, blk, w, feats, scale, side_copy=False):
+    """GPU fused forward + backward through the C ABI; returns host float arrays.
+    side_copy: the forward also writes its float32 copy of O and the backward takes delta from it (bf16 storage)."""
     q, k, v, do = (dev(x, TDT[w.dtype]) for x in feats)
-    O, lse = B.attn_fused_fwd(blk, q, k, v, scale)
-    dQ, dK, dV = B.attn_fused_bwd(blk, q, k, v, O, lse, do, scale)
+    o32 = torch.empty(q.shape, dtype=torch.float32, device=q.device) if side_copy else None
+    O, lse = B.attn_fused_fwd(blk, q, k, v, scale, o32=o32)
+    dQ, dK, dV = B.attn_fused_bwd(blk, q, k, v, O, lse, do, scale, o32=o32)
     torch.cuda.synchronize()
     return tuple(host(x) for x in (O, lse, dQ, dK, dV))
 

@@ -107,16 +107,19 @@ def test_block_build_negative_ids_and_empty(B, oracle_mod):
 # fused forward + backward
 # ------------------------------------------------------------------------------------------------
 
-@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("dtype", ["f32", "bf16", "bf16+o32"])
 @pytest.mark.parametrize("H,D", SHAPES + [(1, 128), (2, 32), (4, 16), (2, 128)])
 def test_fused_small_blocks(B, oracle_mod, H, D, dtype):
-    """degrees 0..40: small + warp tiers, zero-degree rows, ragged group tails."""
+    """degrees 0..40: small + warp tiers, zero-degree rows, ragged group tails.  'bf16+o32': the forward also writes its
+    float32 copy of O and the backward takes delta = <dO, O> from it instead of accumulating it from the edges."""
+    side_copy = dtype.endswith("+o32")
+    dtype = dtype.split("+")[0]
     w = W.small_random(100 + H * D, 500, 40, 120, H, D, dtype=dtype, shuffle=True, zero_frac=0.15)
     ob = _oblock(oracle_mod, w)
     gb = gpu_block(B, w)
     feats = w.features(ob.U)
     scale = 2.0
-    got = run_fused(B, gb, w, feats, scale)
+    got = run_fused(B, gb, w, feats, scale, side_copy=side_copy)
     ref = oracle_fused(oracle_mod, ob, feats, scale)
     for n, g, r in zip(("O", "LSE", "dQ", "dK", "dV"), got, ref):
         assert_close(n, g, r, dtype)
@@ -124,10 +127,12 @@ def test_fused_small_blocks(B, oracle_mod, H, D, dtype):
     assert np.all(got[0][deg == 0] == 0) and np.all(got[2][deg == 0] == 0)      # zero-degree: O = dQ = 0, LSE = -inf
 
 
-@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("dtype", ["f32", "bf16", "bf16+o32"])
 @pytest.mark.parametrize("H,D", SHAPES)
 def test_fused_all_tiers_with_hubs(B, oracle_mod, H, D, dtype):
     """warp tier, multi-chunk destination hubs (partial (m,l,acc) merge) and a hot source row (dK/dV partial merge)."""
+    side_copy = dtype.endswith("+o32")
+    dtype = dtype.split("+")[0]
     w = _hub_workload(7 + H, H, D, dtype)
     ob = _oblock(oracle_mod, w)
     gb = gpu_block(B, w)
@@ -135,7 +140,7 @@ def test_fused_all_tiers_with_hubs(B, oracle_mod, H, D, dtype):
     assert info["dst_slots"] >= 4 and info["src_slots"] >= 2 and info["dst_warp_items"] >= info["dst_slots"]
     feats = w.features(ob.U)
     scale = float(math.sqrt(D))                                              # logits ~ N(0,1): softmax far from uniform
-    got = run_fused(B, gb, w, feats, scale)
+    got = run_fused(B, gb, w, feats, scale, side_copy=side_copy)
     ref = oracle_fused(oracle_mod, ob, feats, scale)
     for n, g, r in zip(("O", "LSE", "dQ", "dK", "dV"), got, ref):
         assert_close(n, g, r, dtype)
