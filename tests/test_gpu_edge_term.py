@@ -59,7 +59,7 @@ def test_edge_term_small_blocks(B, oracle_mod, H, D, dtype, slope):
 
 
 @pytest.mark.parametrize("dtype", ["f32", "bf16"])
-@pytest.mark.parametrize("H,D", [(2, 50), (8, 16)])
+@pytest.mark.parametrize("H,D", [(2, 50), (4, 32), (8, 16), (2, 64)])
 def test_edge_term_with_hubs(B, oracle_mod, H, D, dtype):
     w = _hub_workload(17 + H, H, D, dtype, hub_deg=6000)
     _compare(B, oracle_mod, w, float(math.sqrt(D)), 0.2)
