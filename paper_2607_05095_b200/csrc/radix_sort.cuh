@@ -19,10 +19,10 @@ constexpr int TG_RS_BINS = 1 << TG_RS_BITS;
 constexpr int TG_RS_THREADS = 256;
 constexpr int TG_RS_WARPS = TG_RS_THREADS / 32;
 #ifndef TG_RS_ITEMS32
-#define TG_RS_ITEMS32 16
+#define TG_RS_ITEMS32 8
 #endif
 #ifndef TG_RS_MINB
-#define TG_RS_MINB 3
+#define TG_RS_MINB 4
 #endif
 template <class K> struct RsTile { static constexpr int ITEMS = sizeof(K) == 4 ? TG_RS_ITEMS32 : 12; static constexpr int TILE = TG_RS_THREADS * ITEMS; };
 
@@ -36,12 +36,11 @@ __global__ void __launch_bounds__(TG_RS_THREADS) tg_rs_hist(int64_t n, const K* 
     h[threadIdx.x] = 0;
     __syncthreads();
     const int64_t base = (int64_t)blockIdx.x * TILE;
-    for (int i = threadIdx.x; i < TILE; i += TG_RS_THREADS) {   // TILE is a multiple of the CTA size: warp-uniform trip count
+    // plain shared-memory atomics: warp-aggregating them with __match_any_sync was measured slower (41.7 vs 27.6 us per pass on
+    // config 4), even with a key that holds 18 % of the edges
+    for (int i = threadIdx.x; i < TILE; i += TG_RS_THREADS) {
         const int64_t g = base + i;
-        const bool ok = g < n;
-        const int d = ok ? tg_rs_digit(keys[g], shift) : (TG_RS_BINS + (threadIdx.x & 31));
-        const unsigned peers = __match_any_sync(0xffffffffu, d);     // a hot key would serialise the CTA on one counter
-        if (ok && (threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&h[d], __popc(peers));
+        if (g < n) atomicAdd(&h[tg_rs_digit(keys[g], shift)], 1);
     }
     __syncthreads();
     counts[(int64_t)threadIdx.x * n_tiles + blockIdx.x] = h[threadIdx.x];
