@@ -456,6 +456,64 @@ def run_next34(args, B, blocks, bi_dom, extras, peak):
         extras["sampler"] = out
 
 
+def run_e2e_sampled(args, B, extras):
+    """`--e2e-sampled` (configs 1 and 3): the step end to end the B200-first way: the event stream's T-CSR and
+    the node feature tables live in HBM (config 3: 1 M nodes x 256 B x 2 tables = 0.5 GB of 180 GB), so per step the host
+    sends only the batch's roots (node, cutoff) and the per-root tensors (Q, dO); the sampler, the block build, the
+    K / V row gather (tg_cache_lookup + tg_feature_reconstruct, every row resident) and the fused forward + backward run
+    on the device; O, dQ, dK, dV come back.  No sampled list and no feature row crosses PCIe."""
+    import torch
+    from paper_2607_05095_b200 import workloads as W
+    cid = args.config
+    n_nodes, n_events, batch, k, mode = {1: (20_000, 200_000, 600, 10, "recent"), 3: (1_000_000, 50_000_000, 4000, 20, "uniform")}[cid]
+    H, D, dt = {1: (2, 50, torch.float32), 3: (4, 32, torch.bfloat16)}[cid]
+    u, v, t = W._event_stream(args.seed, cid, n_nodes, n_events)
+    rn, rc = W._batch_roots(u, v, n_nodes, batch, args.seed, cid)
+    g = B.tcsr_build(n_nodes, torch.from_numpy(u.astype(np.int64)).cuda(), torch.from_numpy(v.astype(np.int64)).cuda(), torch.from_numpy(t.astype(np.float32)).cuda())
+    del u, v, t
+    gen = torch.Generator(device="cuda").manual_seed(args.seed)
+    Ktab = (torch.randn(n_nodes, H, D, device="cuda", generator=gen) / math.sqrt(D)).to(dt)      # resident node-level K / V rows
+    Vtab = (torch.randn(n_nodes, H, D, device="cuda", generator=gen) / math.sqrt(D)).to(dt)
+    slot = torch.arange(n_nodes, dtype=torch.int32, device="cuda")                               # every node resident: slot = id
+    none_fresh = torch.empty(0, H, D, dtype=dt, device="cuda")
+    R = len(rn)
+    h_rn, h_rc = torch.from_numpy(rn.astype(np.int64)).pin_memory(), torch.from_numpy(rc.astype(np.int64)).pin_memory()
+    h_q = (torch.randn(R, H, D) / math.sqrt(D)).to(dt).pin_memory()
+    h_do = torch.randn(R, H, D).to(dt).pin_memory()
+    d_rn, d_rc, d_q, d_do = (torch.empty_like(x, device="cuda") for x in (h_rn, h_rc, h_q, h_do))
+    h_out = {}
+
+    def step():
+        for dst, src in ((d_rn, h_rn), (d_rc, h_rc), (d_q, h_q), (d_do, h_do)):
+            dst.copy_(src, non_blocking=True)
+        lists = B.sample_neighbors(g, d_rn, d_rc, k, mode, args.seed)
+        blk = B.block_build(R, lists[0], lists[1], lists[2], lists[3], 1)
+        m_, _ = B.cache_lookup(blk.uniq_node, slot)
+        K = B.feature_reconstruct(None, m_, none_fresh, Ktab)
+        V = B.feature_reconstruct(None, m_, none_fresh, Vtab)
+        O, lse = B.attn_fused_fwd(blk, d_q, K, V, 1.0)
+        dQ, dK, dV = B.attn_fused_bwd(blk, d_q, K, V, O, lse, d_do, 1.0)
+        for n, x in (("O", O), ("dQ", dQ), ("dK", dK), ("dV", dV)):
+            if n not in h_out or h_out[n].shape != x.shape:
+                h_out[n] = torch.empty(x.shape, dtype=x.dtype).pin_memory()
+            h_out[n].copy_(x, non_blocking=True)
+        torch.cuda.synchronize()
+        return blk
+
+    blk = step()
+    n = max(3, min(args.steps, 20))
+    t0 = time.perf_counter()
+    for _ in range(n):
+        blk = step()
+    ms = (time.perf_counter() - t0) * 1e3 / n
+    h2d = sum(x.numel() * x.element_size() for x in (h_rn, h_rc, h_q, h_do))
+    d2h = sum(x.numel() * x.element_size() for x in h_out.values())
+    extras["e2e_sampled"] = {"ms_per_step": ms, "edges": blk.E, "unique_rows": blk.U, "edges_per_s": blk.E / (ms * 1e-3), "h2d_bytes_per_step": h2d,
+                             "d2h_bytes_per_step": d2h, "resident_bytes": int(Ktab.numel() * Ktab.element_size() * 2 + g.nbr.numel() * 20),
+                             "sampling": f"{mode}, k = {k}, on the device", "steps": n,
+                             "note": "host sends roots + Q + dO, receives O, dQ, dK, dV; T-CSR and node-level K / V tables resident in HBM; synchronous steps (no overlap)"}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -700,6 +758,8 @@ def run_ours(args):
     run_extras(args, B, blocks, bi_dom, extras, peak)
     if not args.no_unfused:
         run_next34(args, B, blocks, bi_dom, extras, peak)
+    if args.e2e_sampled and args.config in (1, 3):
+        run_e2e_sampled(args, B, extras)
     extras["kernel_ms"] = kms
     extras["schedule"] = blocks[bi_dom]["info"]
 
@@ -737,6 +797,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-unfused", action="store_true", help="skip the extras: unfused chain, edge term, SlimCache, plain AGG, sampler")
     ap.add_argument("--no-sampler", action="store_true")
+    ap.add_argument("--e2e-sampled", action="store_true", help="configs 1, 3: extras.e2e_sampled = the step with the sampler and the feature rows on the device")
     ap.add_argument("--side-copy", action="store_true", help="bf16 storage: the forward writes a float32 side copy of O, the backward takes delta from it")
     args = ap.parse_args()
     if args.probe_gather:
