@@ -69,19 +69,33 @@ __device__ __forceinline__ void tg_cta_merge(Op& op, float (&st)[Op::NS1], float
     }
 }
 
+// Where an edge loop takes its row indices from: global memory (positions clamped to the row's last edge), or a chunk
+// staged in shared memory by the warp (TG_STAGE_IDX variant of the warp tier; the stage is padded with the last index, so no clamp).
+struct tg_idx_global {
+    const int32_t* __restrict__ p;
+    int last;
+    __device__ __forceinline__ int operator()(int pos) const { return tg_ldg_i32(p + min(pos, last)); }
+};
+struct tg_idx_shared {
+    const int32_t* s;   // s[0] = index of position `base`
+    int base;
+    __device__ __forceinline__ int operator()(int pos) const { return s[pos - base]; }
+};
+constexpr int TG_STAGE_PAD = 64;   // the pipelined loop looks up to 5 trips (5 * U * G <= 40 positions) past the chunk's end
+
 // Plain edge loop of one group: edges pos = i0 + n*stride < end, U per trip, all loads of a trip issued
 // before its arithmetic.  Latency is hidden by the other warps (small register budget).
 template <int U, class Op>
 __device__ __forceinline__ void tg_run_edges_plain(Op& op, float (&st)[Op::NS1], int i0, int end, int stride, int trips) {
     if (trips <= 0) return;
-    const int32_t* __restrict__ idx = op.idx_ptr();
     const int last = max(end - 1, 0);
+    const tg_idx_global idx{op.idx_ptr(), last};
     int pos = i0;
     for (int t = 0; t < trips; ++t) {
         typename Op::Buf A[U];
         int r[U];
 #pragma unroll
-        for (int u = 0; u < U; ++u) r[u] = tg_ldg_i32(idx + min(pos + u * stride, last));
+        for (int u = 0; u < U; ++u) r[u] = idx(pos + u * stride);
 #pragma unroll
         for (int u = 0; u < U; ++u) op.load(A[u], r[u], min(pos + u * stride, last));
         op.template compute<U, true>(st, A, pos, stride, end);
@@ -97,29 +111,28 @@ __device__ __forceinline__ void tg_run_edges_plain(Op& op, float (&st)[Op::NS1],
 // index -> address dependency).  Positions past `end` are clamped for the loads (a valid row is fetched
 // again) and masked in compute().  `full_until`: trips whose first position is below it need no mask
 // (warp-uniform; pass i0 to mask everything).
-template <int U, class Op>
-__device__ __forceinline__ void tg_run_edges_pipe(Op& op, float (&st)[Op::NS1], int i0, int end, int stride, int trips,
-                                                  int full_until) {
+template <int U, class Op, class Idx>
+__device__ __forceinline__ void tg_run_edges_pipe_from(Op& op, float (&st)[Op::NS1], const Idx& idx, int i0, int end, int stride, int trips,
+                                                       int full_until) {
     if (trips <= 0) return;
-    const int32_t* __restrict__ idx = op.idx_ptr();
     const int last = max(end - 1, 0);
     typename Op::Buf A[U], B[U];
     int ia[U], ib[U], na[U], nb[U];   // indices of trips t+2, t+1 (used this iteration) and t+4, t+3 (next one)
     const int step = U * stride;
     int pos = i0;  // first position of the trip being computed
 #pragma unroll
-    for (int u = 0; u < U; ++u) na[u] = tg_ldg_i32(idx + min(pos + u * stride, last));
+    for (int u = 0; u < U; ++u) na[u] = idx(pos + u * stride);
 #pragma unroll
-    for (int u = 0; u < U; ++u) ib[u] = tg_ldg_i32(idx + min(pos + step + u * stride, last));
+    for (int u = 0; u < U; ++u) ib[u] = idx(pos + step + u * stride);
 #pragma unroll
-    for (int u = 0; u < U; ++u) ia[u] = tg_ldg_i32(idx + min(pos + 2 * step + u * stride, last));
+    for (int u = 0; u < U; ++u) ia[u] = idx(pos + 2 * step + u * stride);
 #pragma unroll
     for (int u = 0; u < U; ++u) op.load(A[u], na[u], min(pos + u * stride, last));
     for (int t = 0; t < trips; t += 2) {
 #pragma unroll
-        for (int u = 0; u < U; ++u) nb[u] = tg_ldg_i32(idx + min(pos + 3 * step + u * stride, last));
+        for (int u = 0; u < U; ++u) nb[u] = idx(pos + 3 * step + u * stride);
 #pragma unroll
-        for (int u = 0; u < U; ++u) na[u] = tg_ldg_i32(idx + min(pos + 4 * step + u * stride, last));
+        for (int u = 0; u < U; ++u) na[u] = idx(pos + 4 * step + u * stride);
         if (t + 1 < trips) {
 #pragma unroll
             for (int u = 0; u < U; ++u) op.load(B[u], ib[u], min(pos + step + u * stride, last));
@@ -140,15 +153,23 @@ __device__ __forceinline__ void tg_run_edges_pipe(Op& op, float (&st)[Op::NS1], 
     }
 }
 
+template <int U, class Op>
+__device__ __forceinline__ void tg_run_edges_pipe(Op& op, float (&st)[Op::NS1], int i0, int end, int stride, int trips, int full_until) {
+    tg_run_edges_pipe_from<U>(op, st, tg_idx_global{op.idx_ptr(), max(end - 1, 0)}, i0, end, stride, trips, full_until);
+}
+
 // Warp tier: one warp per item {row, begin, end, slot}.  The warps of a CTA are independent; a CTA holds
 // TG_WARP_CTA_WARPS of them (its registers are released only when its slowest warp ends, so smaller is better
 // for the tail) and MIN_WARPS / TG_WARP_CTA_WARPS such CTAs are resident per SM.
 #ifndef TG_WARP_CTA_WARPS
 #define TG_WARP_CTA_WARPS 1
 #endif
+#ifndef TG_STAGE_IDX
+#define TG_STAGE_IDX 0   // 1: the warp tier of a large side stages its item's index chunk in shared memory (measured, profiles/)
+#endif
 template <class Op, int U, bool PIPE>
 __device__ __forceinline__ void tg_warp_body(const typename Op::Params& p, const int4* __restrict__ items,
-                                             const int32_t* __restrict__ indptr, int n_items, int idx) {
+                                             const int32_t* __restrict__ indptr, int n_items, int idx, int32_t* stage = nullptr) {
     using Tr = typename Op::Tr;
     const int lane = threadIdx.x & 31;
     const int g = lane / Tr::LPR;
@@ -162,7 +183,14 @@ __device__ __forceinline__ void tg_warp_body(const typename Op::Params& p, const
     const int trips = (n + Tr::G * U - 1) / (Tr::G * U);
     // a trip is full for every group when its last position (group G-1, edge U-1) is inside the chunk
     const int full_until = it.y + g + ((n / (Tr::G * U)) * (Tr::G * U));
-    if constexpr (PIPE) tg_run_edges_pipe<U>(op, st, it.y + g, it.z, Tr::G, trips, full_until);
+    if (PIPE && stage != nullptr) {
+        // stage the chunk's indices (+ TG_STAGE_PAD copies of the last one for the loop's look-ahead): coalesced loads once per
+        // item instead of one index load, one clamp and one address computation per edge and trip
+        const int32_t* __restrict__ gi = op.idx_ptr();
+        for (int i = lane; i < n + TG_STAGE_PAD; i += 32) stage[i] = tg_ldg_i32(gi + min(it.y + i, it.z - 1));
+        __syncwarp();
+        tg_run_edges_pipe_from<U>(op, st, tg_idx_shared{stage, it.y}, it.y + g, it.z, Tr::G, trips, full_until);
+    } else if constexpr (PIPE) tg_run_edges_pipe<U>(op, st, it.y + g, it.z, Tr::G, trips, full_until);
     else tg_run_edges_plain<U>(op, st, it.y + g, it.z, Tr::G, trips);
     tg_end_edges(op, st);
     tg_warp_merge(op, st);
@@ -174,7 +202,12 @@ __device__ __forceinline__ void tg_warp_body(const typename Op::Params& p, const
 template <class Op, int U, int MIN_WARPS, bool PIPE>
 __global__ void __launch_bounds__(TG_WARP_CTA_WARPS * 32, MIN_WARPS / TG_WARP_CTA_WARPS) tg_warp_kernel(typename Op::Params p, const int4* __restrict__ items,
                                                                            const int32_t* __restrict__ indptr, int n_items) {
+#if TG_STAGE_IDX
+    __shared__ int32_t sidx[TG_WARP_CTA_WARPS][TG_CHUNK_MAX + TG_STAGE_PAD];
+    tg_warp_body<Op, U, PIPE>(p, items, indptr, n_items, blockIdx.x * TG_WARP_CTA_WARPS + (threadIdx.x >> 5), sidx[threadIdx.x >> 5]);
+#else
     tg_warp_body<Op, U, PIPE>(p, items, indptr, n_items, blockIdx.x * TG_WARP_CTA_WARPS + (threadIdx.x >> 5));
+#endif
 }
 
 // Group tier: one group per record {row, begin, end, 0}; TG_GROUP_CTA_WARPS independent warps per CTA.
