@@ -26,6 +26,15 @@ static inline bool tg_shape_supported(int H, int D, tg_dtype_t dtype) {
     return false;
 }
 
+// Layout override for one kernel: RowTraits with MAXW words per lane if that keeps every partial-state size of the default
+// layout (the workspaces are sized with the default layout), else the default layout.
+template <class Tr0, int MAXW>
+struct tg_relayout {
+    using Alt = RowTraits<typename Tr0::T, Tr0::H, Tr0::D, MAXW>;
+    static constexpr bool same = Alt::NE * Alt::LPR == Tr0::NE * Tr0::LPR && Alt::NHL * Alt::LPR == Tr0::NHL * Tr0::LPR;
+    using type = typename std::conditional<same, Alt, Tr0>::type;
+};
+
 // per-lane geometry for workspace sizing
 struct tg_geom { int NE, LPR, NHL; };
 template <class Tr> struct GeomFn {

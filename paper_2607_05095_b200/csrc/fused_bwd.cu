@@ -61,6 +61,20 @@
 
 template <class X> struct tg_type_tag { using type = X; };
 
+// words of a gathered 256-byte bf16 row per lane: 8 = LPR 8 (two vectors per lane), 4 = LPR 16 (one vector per lane: half the
+// buffer / accumulator registers per thread, the same instructions per edge, 24 instead of 16 resident warps).  Measured on config 4
+// (profiles/r01_other_configs_and_probes.md, round-2 additions): forward 0.367 -> 0.352 ms, destination-major backward 0.475 -> 0.450 ms,
+// source-major backward 0.539 -> 0.592 ms -- so the first two use LPR 16, the source-major pass stays at LPR 8.
+#ifndef TG_BWD1_MAXW
+#define TG_BWD1_MAXW 4
+#endif
+#ifndef TG_BWD1_WARPSW16
+#define TG_BWD1_WARPSW16 24
+#endif
+#ifndef TG_BWD2_MAXW
+#define TG_BWD2_MAXW 8
+#endif
+
 struct BwdArgs {
     const tg_block* b;
     const void *Q, *K, *V, *O, *dO;
@@ -89,7 +103,7 @@ struct BwdFn {
         if (which & 1) {
             // wide fp32 rows: 16 words per lane (LPR 8) and a single gather buffer, as in the source-major pass below
             constexpr bool WIDE1 = !Tr::BF16 && Tr::F * Tr::EB >= 512;
-            using Tr1 = RowTraits<T, Tr::H, Tr::D, WIDE1 ? 16 : 8>;
+            using Tr1 = typename std::conditional<WIDE1, RowTraits<T, Tr::H, Tr::D, 16>, typename tg_relayout<Tr, (Tr::BF16 && Tr::F * Tr::EB == 256) ? TG_BWD1_MAXW : 8>::type>::type;
             auto launch = [&](auto tag) -> tg_status_t {
                 using Op = typename decltype(tag)::type;
                 static_assert(Tr1::NE * Tr1::LPR <= Tr::NE * Tr::LPR, "the partial workspace is sized with the default layout");
@@ -104,7 +118,10 @@ struct BwdFn {
                     return tg_launch_tiers<Op, TierPolicy<1, 2, 1, 2, 1, 16, false>>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst");
                 } else {
                     using OpW = typename tg_warp_op<Op, (TG_BWD1_MMA != 0) && MmaDotOk<Tr1>::value>::type;
-                    return tg_launch_tiers<Op, TierPolicy<TG_BWD1_POLICY>, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst");
+                    if constexpr (Tr1::LPR == 16 && Tr1::BF16)
+                        return tg_launch_tiers<Op, TierPolicy<TG_BWD1_U, TG_BWD1_CTAS, TG_BWD1_UP, TG_BWD1_CTASP, TG_BWD1_UW, TG_BWD1_WARPSW16, TG_BWD1_WPIPE>, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst");
+                    else
+                        return tg_launch_tiers<Op, TierPolicy<TG_BWD1_POLICY>, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst");
                 }
             };
             // bf16 storage: with the forward's fp32 copy of O delta = <dO, O> is taken up front (one accumulator and 16 registers
@@ -115,7 +132,7 @@ struct BwdFn {
         if (which & 2) {
             // wide fp32 rows: 16 words per lane (LPR 8) and a single gather buffer; the lane layout is private to a kernel
             constexpr bool WIDE = !Tr::BF16 && Tr::F * Tr::EB >= 512;
-            using Tr2 = RowTraits<T, Tr::H, Tr::D, WIDE ? 16 : 8>;
+            using Tr2 = typename std::conditional<WIDE, RowTraits<T, Tr::H, Tr::D, 16>, typename tg_relayout<Tr, (Tr::BF16 && Tr::F * Tr::EB == 256) ? TG_BWD2_MAXW : 8>::type>::type;
             using Op = Bwd2Op<Tr2>;
             static_assert(Tr2::NE * Tr2::LPR <= Tr::NE * Tr::LPR, "the partial workspace is sized with the default layout");
             typename Op::Params p;

@@ -44,9 +44,16 @@ struct FwdArgs {
     float* O32;
 };
 
-template <class Tr>
+#ifndef TG_FWD_MAXW
+#define TG_FWD_MAXW 4   // words of a gathered 256-byte bf16 row per lane (8: LPR 8, 4: LPR 16), see fused_bwd.cu
+#endif
+#ifndef TG_FWD_WARPSW16
+#define TG_FWD_WARPSW16 24   // resident warps per SM of the warp tier in the LPR-16 layout (92 registers)
+#endif
+template <class Tr0>
 struct FwdFn {
     static tg_status_t run(const FwdArgs& a) {
+        using Tr = typename tg_relayout<Tr0, (Tr0::BF16 && Tr0::F * Tr0::EB == 256) ? TG_FWD_MAXW : 8>::type;
         using Op = FwdOp<Tr>;
         using OpW = typename tg_warp_op<Op, (TG_FWD_MMA != 0) && MmaDotOk<Tr>::value>::type;
         using T = typename Tr::T;
@@ -58,7 +65,10 @@ struct FwdFn {
         p.part = static_cast<float*>(a.ws);
         p.scale2 = a.scale * TG_LOG2E;
         p.O32 = a.O32;
-        return tg_launch_tiers<Op, TierPolicy<TG_FWD_POLICY>, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_fwd");
+        if constexpr (Tr::LPR == 16 && Tr::BF16)
+            return tg_launch_tiers<Op, TierPolicy<TG_FWD_U, TG_FWD_CTAS, TG_FWD_UP, TG_FWD_CTASP, TG_FWD_UW, TG_FWD_WARPSW16, TG_FWD_WPIPE>, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_fwd");
+        else
+            return tg_launch_tiers<Op, TierPolicy<TG_FWD_POLICY>, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_fwd");
     }
 };
 
