@@ -59,8 +59,6 @@
 #define TG_BWD2_MMA 0
 #endif
 
-template <class X> struct tg_type_tag { using type = X; };
-
 // words of a gathered 256-byte bf16 row per lane: 8 = LPR 8 (two vectors per lane), 4 = LPR 16 (one vector per lane: half the
 // buffer / accumulator registers per thread, the same instructions per edge, 24 instead of 16 resident warps).  Measured on config 4
 // (profiles/r01_other_configs_and_probes.md, round-2 additions): forward 0.367 -> 0.352 ms, destination-major backward 0.475 -> 0.450 ms,
@@ -70,6 +68,23 @@ template <class X> struct tg_type_tag { using type = X; };
 #endif
 #ifndef TG_BWD1_WARPSW16
 #define TG_BWD1_WARPSW16 24
+#endif
+#ifndef TG_BWD2_WARPSW16
+#define TG_BWD2_WARPSW16 24
+#endif
+// fp32 rows of 512 bytes: 16 = the wide single-buffered layout (LPR 8), 8 = LPR 16, 4 = LPR 32, both pipelined.  Measured on config 5:
+// destination-major 6.92 (wide) / 7.69 (LPR 16) / 6.43 ms (LPR 32); source-major 6.20 (wide) / 8.06 / 7.90 ms
+#ifndef TG_BWD1_MAXW_F32
+#define TG_BWD1_MAXW_F32 4
+#endif
+#ifndef TG_BWD2_MAXW_F32
+#define TG_BWD2_MAXW_F32 16
+#endif
+#ifndef TG_BWD1_GROUP_RELAYOUT
+#define TG_BWD1_GROUP_RELAYOUT 1   // 1: the group tiers use the warp tier's layout too
+#endif
+#ifndef TG_BWD2_GROUP_RELAYOUT
+#define TG_BWD2_GROUP_RELAYOUT 0
 #endif
 #ifndef TG_BWD2_MAXW
 #define TG_BWD2_MAXW 8
@@ -100,13 +115,20 @@ struct BwdFn {
         float* dq_part = static_cast<float*>(c.take(sz.dq_part));
         float* dkv_part = static_cast<float*>(c.take(sz.dkv_part));
         if (!c.ok()) TG_FAIL(TG_ERR_WORKSPACE, "fused bwd needs %zu workspace bytes", c.off);
+        // Lane layouts (rowops.cuh): wide fp32 rows run at 16 words per lane, single-buffered; bf16 rows of 256 bytes run their WARP
+        // tier (and the hub merges that read its partials) at 4 words per lane (LPR 16) where that was measured faster, their group
+        // tiers in the default layout (LPR 8: four rows per warp instruction).  The layout is private to a launch.
+        constexpr bool F512 = !Tr::BF16 && Tr::F * Tr::EB == 512;
+        constexpr bool B256 = Tr::BF16 && Tr::F * Tr::EB == 256;
         if (which & 1) {
-            // wide fp32 rows: 16 words per lane (LPR 8) and a single gather buffer, as in the source-major pass below
-            constexpr bool WIDE1 = !Tr::BF16 && Tr::F * Tr::EB >= 512;
-            using Tr1 = typename std::conditional<WIDE1, RowTraits<T, Tr::H, Tr::D, 16>, typename tg_relayout<Tr, (Tr::BF16 && Tr::F * Tr::EB == 256) ? TG_BWD1_MAXW : 8>::type>::type;
+            constexpr bool WIDE = !Tr::BF16 && Tr::F * Tr::EB >= 512 && !(F512 && TG_BWD1_MAXW_F32 != 16);
+            using TrW = typename std::conditional<WIDE, RowTraits<T, Tr::H, Tr::D, 16>, typename tg_relayout<Tr, B256 ? TG_BWD1_MAXW : F512 ? TG_BWD1_MAXW_F32 : 8>::type>::type;
+            using TrG = typename std::conditional<WIDE || TG_BWD1_GROUP_RELAYOUT != 0, TrW, Tr>::type;
+            static_assert(TrW::NE * TrW::LPR <= Tr::NE * Tr::LPR, "the partial workspace is sized with the default layout");
             auto launch = [&](auto tag) -> tg_status_t {
-                using Op = typename decltype(tag)::type;
-                static_assert(Tr1::NE * Tr1::LPR <= Tr::NE * Tr::LPR, "the partial workspace is sized with the default layout");
+                constexpr bool ED = decltype(tag)::value;      // delta from the edges (bf16 without the fp32 copy of O)
+                using Op = Bwd1Op<TrG, ED>;
+                using OpW0 = Bwd1Op<TrW, ED>;
                 typename Op::Params p;
                 p.Q = static_cast<const T*>(a.Q); p.K = static_cast<const T*>(a.K); p.V = static_cast<const T*>(a.V);
                 p.O = static_cast<const T*>(a.O); p.dO = static_cast<const T*>(a.dO);
@@ -114,11 +136,11 @@ struct BwdFn {
                 p.dQ = static_cast<T*>(a.dQ); p.ld = ld; p.part = dq_part;
                 p.scale = a.scale; p.scale2 = a.scale * TG_LOG2E;
                 p.O32 = a.O32;
-                if constexpr (WIDE1) {
-                    return tg_launch_tiers<Op, TierPolicy<1, 2, 1, 2, 1, 16, false>>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst");
+                if constexpr (WIDE) {
+                    return tg_launch_tiers<Op, TierPolicy<1, 2, 1, 2, 1, 16, false>, OpW0>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst");
                 } else {
-                    using OpW = typename tg_warp_op<Op, (TG_BWD1_MMA != 0) && MmaDotOk<Tr1>::value>::type;
-                    if constexpr (Tr1::LPR == 16 && Tr1::BF16)
+                    using OpW = typename tg_warp_op<OpW0, (TG_BWD1_MMA != 0) && ED == Tr::BF16 && MmaDotOk<TrW>::value>::type;
+                    if constexpr ((TrW::LPR == 16 && TrW::BF16) || (TrW::LPR == 32 && !TrW::BF16 && TrW::NW == 4))
                         return tg_launch_tiers<Op, TierPolicy<TG_BWD1_U, TG_BWD1_CTAS, TG_BWD1_UP, TG_BWD1_CTASP, TG_BWD1_UW, TG_BWD1_WARPSW16, TG_BWD1_WPIPE>, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst");
                     else
                         return tg_launch_tiers<Op, TierPolicy<TG_BWD1_POLICY>, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst");
@@ -126,26 +148,30 @@ struct BwdFn {
             };
             // bf16 storage: with the forward's fp32 copy of O delta = <dO, O> is taken up front (one accumulator and 16 registers
             // fewer per lane); without it delta is accumulated from the edges
-            if (Tr::BF16 && a.O32) TG_TRY(launch(tg_type_tag<Bwd1Op<Tr1, false>>{}));
-            else TG_TRY(launch(tg_type_tag<Bwd1Op<Tr1>>{}));
+            if (Tr::BF16 && !a.O32) TG_TRY(launch(std::true_type{}));
+            else TG_TRY(launch(std::false_type{}));
         }
         if (which & 2) {
-            // wide fp32 rows: 16 words per lane (LPR 8) and a single gather buffer; the lane layout is private to a kernel
-            constexpr bool WIDE = !Tr::BF16 && Tr::F * Tr::EB >= 512;
-            using Tr2 = typename std::conditional<WIDE, RowTraits<T, Tr::H, Tr::D, 16>, typename tg_relayout<Tr, (Tr::BF16 && Tr::F * Tr::EB == 256) ? TG_BWD2_MAXW : 8>::type>::type;
-            using Op = Bwd2Op<Tr2>;
-            static_assert(Tr2::NE * Tr2::LPR <= Tr::NE * Tr::LPR, "the partial workspace is sized with the default layout");
+            constexpr bool WIDE = !Tr::BF16 && Tr::F * Tr::EB >= 512 && !(F512 && TG_BWD2_MAXW_F32 != 16);
+            using TrW = typename std::conditional<WIDE, RowTraits<T, Tr::H, Tr::D, 16>, typename tg_relayout<Tr, B256 ? TG_BWD2_MAXW : F512 ? TG_BWD2_MAXW_F32 : 8>::type>::type;
+            using TrG = typename std::conditional<WIDE || TG_BWD2_GROUP_RELAYOUT != 0, TrW, Tr>::type;
+            static_assert(TrW::NE * TrW::LPR <= Tr::NE * Tr::LPR, "the partial workspace is sized with the default layout");
+            using Op = Bwd2Op<TrG>;
+            using OpW0 = Bwd2Op<TrW>;
             typename Op::Params p;
             p.Q = static_cast<const T*>(a.Q); p.K = static_cast<const T*>(a.K); p.V = static_cast<const T*>(a.V);
             p.dO = static_cast<const T*>(a.dO);
             p.t_dst = a.b->t_dst; p.ld = ld;
             p.dK = static_cast<T*>(a.dK); p.dV = static_cast<T*>(a.dV); p.part = dkv_part;
             p.scale = a.scale; p.scale2 = a.scale * TG_LOG2E;
-            if constexpr (WIDE)
-                TG_TRY((tg_launch_tiers<Op, TierPolicy<1, 2, 1, 2, 1, 16, false>>(p, a.b->src, a.stream, "tg_attn_fused_bwd/src")));
-            else {
-                using OpW = typename tg_warp_op<Op, (TG_BWD2_MMA != 0) && MmaDotOk<Tr2>::value>::type;
-                TG_TRY((tg_launch_tiers<Op, TierPolicy<TG_BWD2_POLICY>, OpW>(p, a.b->src, a.stream, "tg_attn_fused_bwd/src")));
+            if constexpr (WIDE) {
+                TG_TRY((tg_launch_tiers<Op, TierPolicy<1, 2, 1, 2, 1, 16, false>, OpW0>(p, a.b->src, a.stream, "tg_attn_fused_bwd/src")));
+            } else {
+                using OpW = typename tg_warp_op<OpW0, (TG_BWD2_MMA != 0) && MmaDotOk<TrW>::value>::type;
+                if constexpr ((TrW::LPR == 16 && TrW::BF16) || (TrW::LPR == 32 && !TrW::BF16 && TrW::NW == 4))
+                    TG_TRY((tg_launch_tiers<Op, TierPolicy<TG_BWD2_U, TG_BWD2_CTAS, TG_BWD2_UP, TG_BWD2_CTASP, TG_BWD2_UW, TG_BWD2_WARPSW16, TG_BWD2_WPIPE>, OpW>(p, a.b->src, a.stream, "tg_attn_fused_bwd/src")));
+                else
+                    TG_TRY((tg_launch_tiers<Op, TierPolicy<TG_BWD2_POLICY>, OpW>(p, a.b->src, a.stream, "tg_attn_fused_bwd/src")));
             }
         }
         return TG_OK;

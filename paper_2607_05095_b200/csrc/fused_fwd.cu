@@ -44,8 +44,14 @@ struct FwdArgs {
     float* O32;
 };
 
+#ifndef TG_FWD_GROUP_RELAYOUT
+#define TG_FWD_GROUP_RELAYOUT 1   // 1: the group tiers use the warp tier's layout too (config 3: 53.4 -> 51.3 us; config 4 indifferent)
+#endif
 #ifndef TG_FWD_MAXW
 #define TG_FWD_MAXW 4   // words of a gathered 256-byte bf16 row per lane (8: LPR 8, 4: LPR 16), see fused_bwd.cu
+#endif
+#ifndef TG_FWD_MAXW_F32
+#define TG_FWD_MAXW_F32 4   // the same knob for fp32 rows of 512 bytes: 4 = LPR 32 (config 5: forward 5.98 -> 5.36 ms), 8 = LPR 16
 #endif
 #ifndef TG_FWD_WARPSW16
 #define TG_FWD_WARPSW16 24   // resident warps per SM of the warp tier in the LPR-16 layout (92 registers)
@@ -53,10 +59,13 @@ struct FwdArgs {
 template <class Tr0>
 struct FwdFn {
     static tg_status_t run(const FwdArgs& a) {
-        using Tr = typename tg_relayout<Tr0, (Tr0::BF16 && Tr0::F * Tr0::EB == 256) ? TG_FWD_MAXW : 8>::type;
-        using Op = FwdOp<Tr>;
-        using OpW = typename tg_warp_op<Op, (TG_FWD_MMA != 0) && MmaDotOk<Tr>::value>::type;
-        using T = typename Tr::T;
+        // group tiers: default layout (LPR 8: four rows per warp instruction); warp tier + hub merges: bf16 rows of 256 bytes in the
+        // LPR-16 layout (one vector per lane, half the buffer / accumulator registers, 24 resident warps)
+        using TrW = typename tg_relayout<Tr0, (Tr0::BF16 && Tr0::F * Tr0::EB == 256) ? TG_FWD_MAXW : (!Tr0::BF16 && Tr0::F * Tr0::EB == 512) ? TG_FWD_MAXW_F32 : 8>::type;
+        using TrG = typename std::conditional<TG_FWD_GROUP_RELAYOUT != 0, TrW, Tr0>::type;
+        using Op = FwdOp<TrG>;
+        using OpW = typename tg_warp_op<FwdOp<TrW>, (TG_FWD_MMA != 0) && MmaDotOk<TrW>::value>::type;
+        using T = typename Tr0::T;
         typename Op::Params p;
         p.Q = static_cast<const T*>(a.Q); p.K = static_cast<const T*>(a.K); p.V = static_cast<const T*>(a.V);
         p.kv = a.b->kv_row;
@@ -65,7 +74,7 @@ struct FwdFn {
         p.part = static_cast<float*>(a.ws);
         p.scale2 = a.scale * TG_LOG2E;
         p.O32 = a.O32;
-        if constexpr (Tr::LPR == 16 && Tr::BF16)
+        if constexpr ((TrW::LPR == 16 && TrW::BF16) || (TrW::LPR == 32 && !TrW::BF16 && TrW::NW == 4))
             return tg_launch_tiers<Op, TierPolicy<TG_FWD_U, TG_FWD_CTAS, TG_FWD_UP, TG_FWD_CTASP, TG_FWD_UW, TG_FWD_WARPSW16, TG_FWD_WPIPE>, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_fwd");
         else
             return tg_launch_tiers<Op, TierPolicy<TG_FWD_POLICY>, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_fwd");

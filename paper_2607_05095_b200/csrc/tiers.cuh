@@ -21,6 +21,8 @@
 //   write_final(row, st, first), write_partial(slot, st, first), load_partial(slot, st)
 // Every warp-wide call (compute, merge) is reached by all 32 lanes with warp-uniform trip counts.
 #pragma once
+#include <string.h>
+
 #include <type_traits>
 
 #include "rowops.cuh"
@@ -243,11 +245,11 @@ __global__ void __launch_bounds__(TG_GROUP_CTA_WARPS * 32, MIN_CTAS * 8 / TG_GRO
 // Small sides (< TG_FORK_MIN_EDGES edges: the K <= 10-20 blocks of configs 1-3) are launch-latency bound: one launch
 // covers the warp tier and both group tiers, 2 independent warps per CTA, blockIdx selects the tier (largest work first).
 template <class Op, class OpW, int UW, int UB, int US, bool WARP_PIPE>
-__global__ void __launch_bounds__(64, 8) tg_small_side_kernel(typename Op::Params p, const int4* __restrict__ items, const int32_t* __restrict__ indptr,
+__global__ void __launch_bounds__(64, 8) tg_small_side_kernel(typename Op::Params p, typename OpW::Params pw, const int4* __restrict__ items, const int32_t* __restrict__ indptr,
                                                               int n_items, const int4* __restrict__ rows, int n_big, int n_small, int nb_items, int nb_big) {
     const int warp = threadIdx.x >> 5;
     int b = blockIdx.x;
-    if (b < nb_items) { tg_warp_body<OpW, UW, WARP_PIPE>(p, items, indptr, n_items, b * 2 + warp); return; }
+    if (b < nb_items) { tg_warp_body<OpW, UW, WARP_PIPE>(pw, items, indptr, n_items, b * 2 + warp); return; }
     b -= nb_items;
     if (b < nb_big) { tg_group_body<Op, UB, WARP_PIPE>(p, rows, n_big, b * 2 + warp); return; }
     b -= nb_big;
@@ -374,7 +376,12 @@ static tg_status_t tg_launch_hub_merge(const typename Op::Params& p, const tg_si
 // OpW: the operator of the warp tier (same Params, same state layout outside the edge loop; e.g. the HMMA variants of ops_mma.cuh).
 template <class Op, class Pol, class OpW = Op>
 static tg_status_t tg_launch_tiers(const typename Op::Params& p, const tg_side& s, cudaStream_t stream, const char* name) {
-    static_assert(std::is_same<typename Op::Params, typename OpW::Params>::value && Op::NS == OpW::NS, "warp-tier operator must share Params and state");
+    // The warp tier (and the hub merges, which read its partials) may run the operator in another lane layout than the group
+    // tiers: Params hold only pointers and scalars, field for field the same whatever the layout.
+    static_assert(sizeof(typename Op::Params) == sizeof(typename OpW::Params) && std::is_trivially_copyable<typename Op::Params>::value &&
+                      std::is_trivially_copyable<typename OpW::Params>::value, "warp-tier operator must share the Params fields");
+    typename OpW::Params pw;
+    memcpy(&pw, &p, sizeof(pw));
     using Tr = typename Op::Tr;
     if (s.n_rows == 0) return TG_OK;
     constexpr int rows_per_cta = TG_GROUP_CTA_WARPS * Tr::G;
@@ -383,10 +390,10 @@ static tg_status_t tg_launch_tiers(const typename Op::Params& p, const tg_side& 
         const int nb_items = (s.n_items + 1) / 2, nb_big = (n_big + 2 * Tr::G - 1) / (2 * Tr::G), nb_small = (n_small + 2 * Tr::G - 1) / (2 * Tr::G);
         if (nb_items + nb_big + nb_small > 0) {
             tg_small_side_kernel<Op, OpW, Pol::U_WARP, Pol::U_PIPE, Pol::U_PLAIN, Pol::WARP_PIPE><<<(unsigned)(nb_items + nb_big + nb_small), 64, 0, stream>>>(
-                p, s.items, s.indptr, s.n_items, s.rows, n_big, n_small, nb_items, nb_big);
+                p, pw, s.items, s.indptr, s.n_items, s.rows, n_big, n_small, nb_items, nb_big);
             TG_LAUNCH_CHECK(name);
         }
-        if constexpr (Op::NS > 0) TG_TRY((tg_launch_hub_merge<Op>(p, s, stream, name)));
+        if constexpr (Op::NS > 0) TG_TRY((tg_launch_hub_merge<OpW>(pw, s, stream, name)));
         return TG_OK;
     }
     const bool fork = s.n_items > 0 && (n_big > 0 || n_small > 0);
@@ -403,7 +410,7 @@ static tg_status_t tg_launch_tiers(const typename Op::Params& p, const tg_side& 
     auto launch_all = [&]() -> tg_status_t {
         if (s.n_items > 0) {
             const unsigned grid = (unsigned)((s.n_items + TG_WARP_CTA_WARPS - 1) / TG_WARP_CTA_WARPS);
-            tg_warp_kernel<OpW, Pol::U_WARP, Pol::WARPS_WARP, Pol::WARP_PIPE><<<grid, TG_WARP_CTA_WARPS * 32, 0, stream>>>(p, s.items, s.indptr, s.n_items);
+            tg_warp_kernel<OpW, Pol::U_WARP, Pol::WARPS_WARP, Pol::WARP_PIPE><<<grid, TG_WARP_CTA_WARPS * 32, 0, stream>>>(pw, s.items, s.indptr, s.n_items);
             TG_LAUNCH_CHECK(name);
         }
         if (n_big > 0) {
@@ -420,7 +427,7 @@ static tg_status_t tg_launch_tiers(const typename Op::Params& p, const tg_side& 
             tg_group_kernel<Op, Pol::U_PLAIN, Pol::CTAS_PLAIN, false><<<grid, TG_GROUP_CTA_WARPS * 32, 0, sx>>>(p, s.rows + n_big, n_small);
             TG_LAUNCH_CHECK(name);
         }
-        if constexpr (Op::NS > 0) TG_TRY((tg_launch_hub_merge<Op>(p, s, stream, name)));
+        if constexpr (Op::NS > 0) TG_TRY((tg_launch_hub_merge<OpW>(pw, s, stream, name)));
         return TG_OK;
     };
     st = launch_all();
