@@ -312,6 +312,27 @@ TG_API tg_status_t tg_cache_lookup(int64_t U, const int64_t* uniq_ids, const int
 TG_API tg_status_t tg_feature_reconstruct(int64_t n, int64_t row_bytes, const int32_t* inv_idx, const int32_t* map,
                                           const void* fresh_rows, const void* cache_rows, void* out, tg_stream_t stream);
 
+/* tg_cache_lookup for callers that cannot provide a workspace because they cannot allocate device memory at this point:
+ * a serving process whose memory pool is fixed and fully assigned, a plug-in that receives tensors from a host framework
+ * but has no allocator of its own, a latency-critical thread that must stay clear of cudaMalloc (which serialises the
+ * device).  Same inputs, outputs and results as tg_cache_lookup; the scan's scratch is a fixed array inside the library
+ * image instead of `ws`.
+ *   Limit.    U <= TG_CACHE_STATIC_MAX_IDS (2^22 unique ids per call); a larger U returns TG_ERR_WORKSPACE with a message
+ *             and launches nothing -- use tg_cache_lookup there.  The array is about 17 KB and stays resident on every GPU
+ *             that uses this library, from first use until the process exits.
+ *   Allocation. The call performs no cudaMalloc / cudaFree and calls no allocating library routine.
+ *   First call. The first call on each device (with that device current) asks the runtime for the array's device address
+ *             and caches it; make that first call outside any stream capture.  Later calls on the device only launch.
+ *   Sharing.  Every call on a device uses the same array, whatever the stream or thread.  Nothing in it has to be cleared
+ *             between calls (each call overwrites what it later reads), but two calls whose kernels may run at the same
+ *             time on one GPU race on it: keep calls on one device ordered (one stream, or events between streams).  The
+ *             call itself ends with a stream synchronisation, like tg_cache_lookup, so back-to-back calls from one
+ *             thread are already ordered.
+ * Errors: as tg_cache_lookup, plus TG_ERR_WORKSPACE (U beyond the limit) and TG_ERR_UNSUPPORTED (device ordinal >= 64). */
+#define TG_CACHE_STATIC_MAX_IDS (1 << 22)
+TG_API tg_status_t tg_cache_lookup_static(int64_t U, const int64_t* uniq_ids, const int32_t* slot_of_id, int32_t* map,
+                                          int64_t* fresh_ids, int64_t* n_fresh_host /*HOST*/, tg_stream_t stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -26,7 +26,7 @@ EXPORTS = [
     "tg_sddmm", "tg_edge_softmax_fwd", "tg_edge_softmax_bwd", "tg_aggregate_fwd", "tg_aggregate_bwd",
     "tg_attn_workspace_bytes", "tg_attn_fused_fwd", "tg_attn_fused_bwd", "tg_attn_fused_bwd_dst", "tg_attn_fused_bwd_src",
     "tg_attn_edge_fused_fwd", "tg_attn_edge_fused_bwd",
-    "tg_cache_greedy_select", "tg_cache_lookup_workspace_bytes", "tg_cache_lookup", "tg_feature_reconstruct",
+    "tg_cache_greedy_select", "tg_cache_lookup_workspace_bytes", "tg_cache_lookup", "tg_cache_lookup_static", "tg_feature_reconstruct",
     "tg_block_coo_dst", "tg_aggregate_coo",
     "tg_tcsr_workspace_bytes", "tg_tcsr_build", "tg_sample_workspace_bytes", "tg_sample_neighbors",
 ]
@@ -379,6 +379,26 @@ def cache_lookup(uniq_ids: torch.Tensor, slot_of_id: torch.Tensor):
     _check(lib().tg_cache_lookup(C.c_int64(U), _ptr(uniq_ids.contiguous()), _ptr(slot_of_id.contiguous()), _ptr(m), _ptr(fresh), C.byref(n),
                                  _ptr(ws), C.c_size_t(nb.value), _stream()), "tg_cache_lookup")
     return m, fresh[:n.value]
+
+
+CACHE_STATIC_MAX_IDS = 1 << 22   # TG_CACHE_STATIC_MAX_IDS of include/fasttg.h
+
+
+def cache_lookup_static(uniq_ids: torch.Tensor, slot_of_id: torch.Tensor, map_out: torch.Tensor, fresh_out: torch.Tensor):
+    """tg_cache_lookup_static: tg_cache_lookup without a workspace, for callers that must not allocate device memory
+    (fixed memory pool, no allocator of their own, no cudaMalloc on the serving thread).  The caller passes both outputs
+    (map_out int32 [>= U], fresh_out int64 [>= U]); nothing is allocated here or in the library.  Returns n_fresh; the
+    valid results are map_out[:U] and fresh_out[:n_fresh].  U <= CACHE_STATIC_MAX_IDS, else FastTGError (TG_ERR_WORKSPACE).
+    Calls on one device share the library's built-in scratch and must not overlap on the GPU."""
+    U = int(uniq_ids.shape[0])
+    if not (uniq_ids.is_contiguous() and slot_of_id.is_contiguous() and map_out.is_contiguous() and fresh_out.is_contiguous()):
+        raise ValueError("cache_lookup_static: tensors must be contiguous (a copy would allocate)")
+    if map_out.dtype != torch.int32 or fresh_out.dtype != torch.int64 or map_out.numel() < U or fresh_out.numel() < U:
+        raise ValueError("cache_lookup_static: map_out int32 [>= U] and fresh_out int64 [>= U] are required")
+    n = C.c_int64(0)
+    _check(lib().tg_cache_lookup_static(C.c_int64(U), _ptr(uniq_ids), _ptr(slot_of_id), _ptr(map_out), _ptr(fresh_out), C.byref(n),
+                                        _stream()), "tg_cache_lookup_static")
+    return int(n.value)
 
 
 def feature_reconstruct(inv_idx, map_: torch.Tensor, fresh_rows: torch.Tensor, cache_rows: torch.Tensor, out: torch.Tensor | None = None):

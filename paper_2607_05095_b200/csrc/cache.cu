@@ -5,6 +5,7 @@
 //   tg_feature_reconstruct  X[i] = row of occurrence i, through the inverse index, from the transferred rows or the resident
 //                           cache.  DEVICE, a pure HBM gather/copy: 16-byte vectors, consecutive lanes on consecutive vectors.
 #include <algorithm>
+#include <mutex>
 #include <numeric>
 #include <vector>
 
@@ -151,5 +152,71 @@ extern "C" tg_status_t tg_feature_reconstruct(int64_t n, int64_t row_bytes, cons
         k_reconstruct<uint32_t><<<(unsigned)grid, 256, 0, stream>>>(n, vpr, inv_idx, map, static_cast<const uint32_t*>(fresh_rows),
                                                                      static_cast<const uint32_t*>(cache_rows), static_cast<uint32_t*>(out));
     TG_LAUNCH_CHECK("tg_feature_reconstruct");
+    return TG_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// tg_cache_lookup_static: the lookup above for callers that have no way to hand over a workspace.
+//
+// Who that is: code that runs where device allocation is forbidden or impossible -- a serving loop whose memory pool was
+// sized once and is now full by design, a plug-in that is handed tensors by a host framework but owns no allocator, a
+// real-time thread that must not take the driver's allocation lock (cudaMalloc synchronises the whole device).  For them
+// the scan's scratch (one partial sum per tile of 1024 ids plus the grand total) lives in the array below: it is part of
+// the library image, so every GPU on which the library is used holds these ~17 KB from the first use until the process
+// exits, and no call ever asks the driver for memory.
+//
+// `g_lookup_scratch` is a DEVICE object.  In host code the name only identifies the symbol -- it is not an address a
+// kernel can use -- so the address on each device is asked for once (cudaGetSymbolAddress, with that device current) and
+// cached per device ordinal.
+// ---------------------------------------------------------------------------------------------
+constexpr size_t TG_LOOKUP_SCRATCH_TOTAL_OFF = (((size_t)(TG_CACHE_STATIC_MAX_IDS / TG_SCAN_TILE) + 1) * sizeof(IVec<1>) + 255) / 256 * 256 + 256;
+constexpr size_t TG_LOOKUP_SCRATCH_BYTES = TG_LOOKUP_SCRATCH_TOTAL_OFF + 256;   // tile sums (tg_scan_bytes<1>(max)) + the total
+static_assert(TG_CACHE_STATIC_MAX_IDS % TG_SCAN_TILE == 0, "the scratch is sized in whole scan tiles");
+
+static __device__ __align__(256) unsigned char g_lookup_scratch[TG_LOOKUP_SCRATCH_BYTES];
+
+constexpr int TG_MAX_DEVICES = 64;
+static void* g_lookup_scratch_ptr[TG_MAX_DEVICES];   // device address of g_lookup_scratch, per device ordinal (0 = not asked yet)
+static std::mutex g_lookup_scratch_mutex;
+
+// Device address of the scratch on the CURRENT device; the first call per device asks the runtime (this may load the
+// library's device code onto that GPU, which is why it should not happen for the first time inside a stream capture).
+static tg_status_t lookup_scratch_on_current_device(unsigned char** out) {
+    int dev = -1;
+    TG_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= TG_MAX_DEVICES) TG_FAIL(TG_ERR_UNSUPPORTED, "tg_cache_lookup_static: device ordinal %d outside [0, %d)", dev, TG_MAX_DEVICES);
+    std::lock_guard<std::mutex> lock(g_lookup_scratch_mutex);
+    if (!g_lookup_scratch_ptr[dev]) {
+        void* p = nullptr;
+        TG_CUDA(cudaGetSymbolAddress(&p, g_lookup_scratch));
+        if (!p) TG_FAIL(TG_ERR_INTERNAL, "tg_cache_lookup_static: the runtime returned a null address for the scratch symbol");
+        g_lookup_scratch_ptr[dev] = p;
+    }
+    *out = static_cast<unsigned char*>(g_lookup_scratch_ptr[dev]);
+    return TG_OK;
+}
+
+extern "C" tg_status_t tg_cache_lookup_static(int64_t U, const int64_t* uniq_ids, const int32_t* slot_of_id, int32_t* map,
+                                              int64_t* fresh_ids, int64_t* n_fresh_host, tg_stream_t stream_) {
+    if (U < 0 || !n_fresh_host) TG_FAIL(TG_ERR_INVALID_ARG, "tg_cache_lookup_static: bad argument");
+    *n_fresh_host = 0;
+    if (U > (int64_t)TG_CACHE_STATIC_MAX_IDS)
+        TG_FAIL(TG_ERR_WORKSPACE, "tg_cache_lookup_static: U = %lld exceeds the built-in scratch (TG_CACHE_STATIC_MAX_IDS = %lld ids); "
+                                  "use tg_cache_lookup with a caller workspace", (long long)U, (long long)TG_CACHE_STATIC_MAX_IDS);
+    if (U == 0) return TG_OK;
+    if (!uniq_ids || !slot_of_id || !map || !fresh_ids) TG_FAIL(TG_ERR_INVALID_ARG, "tg_cache_lookup_static: null array");
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    unsigned char* scratch = nullptr;
+    TG_TRY(lookup_scratch_on_current_device(&scratch));
+    // Nothing in the scratch has to start at zero: the reduce launch writes every tile sum the spine reads, and the spine
+    // writes the total before anyone reads it, so whatever the previous call left behind is overwritten first.
+    void* tmp = scratch;
+    int* total = reinterpret_cast<int*>(scratch + TG_LOOKUP_SCRATCH_TOTAL_OFF);
+    TG_TRY((tg_scan<1>(U, MissIn{uniq_ids, slot_of_id}, MissOut{uniq_ids, slot_of_id, map, fresh_ids}, tmp,
+                       reinterpret_cast<IVec<1>*>(total), stream)));
+    int n = 0;
+    TG_CUDA(cudaMemcpyAsync(&n, total, 4, cudaMemcpyDeviceToHost, stream));
+    TG_CUDA(cudaStreamSynchronize(stream));
+    *n_fresh_host = n;
     return TG_OK;
 }
