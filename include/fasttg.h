@@ -135,8 +135,17 @@ TG_API tg_status_t tg_block_destroy(tg_block_t* b);
 
 /* Sizes and schedule statistics of a block (HOST outputs; any may be null).
  * stats[0..7] = dst side {group-tier rows with degree <= 8, group-tier rows with degree 9..64, warp-tier
- * chunk items (rows with degree > 64, one per <= 512 edges), partial slots of multi-chunk rows}, src side the same. */
+ * chunk items (rows above the side's group_max, one per `chunk` edges: tg_block_sched_info), partial slots of multi-chunk rows}, src side the same. */
 TG_API tg_status_t tg_block_info(const tg_block_t* b, int64_t* R, int64_t* E, int64_t* U, int64_t stats[8]);
+
+/* Schedule parameters of a block (HOST output): out[0..3] = destination side {group_max: rows of up to this many edges
+ * are group-tier rows, chunk: edges per warp-tier item, number of hub rows (rows split over several items), largest
+ * degree (0 unless some row has more than 8 edges)}, out[4..7] = the source side likewise. */
+TG_API tg_status_t tg_block_sched_info(const tg_block_t* b, int64_t out[8]);
+/* Number of block builds in this process that ran twice because the calling thread's speculation (sorted input, key
+ * width) was too optimistic.  The speculation is sticky (it follows the largest recent need and relaxes after eight
+ * consecutive smaller builds), so a steady workload shows at most one retry per thread and change of regime. */
+TG_API unsigned long long tg_block_build_retries(void);
 
 /* ------------------------------------------------------------------------------------------------
  * Temporal neighbour sampler on the device

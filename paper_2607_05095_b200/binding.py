@@ -19,17 +19,51 @@ _lib = None
 TG_F32, TG_BF16 = 0, 1
 _DTYPES = {torch.float32: TG_F32, torch.bfloat16: TG_BF16}
 
-EXPORTS = [
-    "tg_status_string", "tg_last_error", "tg_version", "tg_supported", "tg_launch_count", "tg_probe_gather",
-    "tg_block_workspace_bytes", "tg_block_build", "tg_sched_workspace_bytes", "tg_block_from_csr",
-    "tg_block_destroy", "tg_block_info",
-    "tg_sddmm", "tg_edge_softmax_fwd", "tg_edge_softmax_bwd", "tg_aggregate_fwd", "tg_aggregate_bwd",
-    "tg_attn_workspace_bytes", "tg_attn_fused_fwd", "tg_attn_fused_bwd", "tg_attn_fused_bwd_dst", "tg_attn_fused_bwd_src",
-    "tg_attn_edge_fused_fwd", "tg_attn_edge_fused_bwd",
-    "tg_cache_greedy_select", "tg_cache_lookup_workspace_bytes", "tg_cache_lookup", "tg_cache_lookup_static", "tg_feature_reconstruct",
-    "tg_block_coo_dst", "tg_aggregate_coo",
-    "tg_tcsr_workspace_bytes", "tg_tcsr_build", "tg_sample_workspace_bytes", "tg_sample_neighbors",
-]
+# Signature of every export of include/fasttg.h: name -> (result, arguments), one letter per C type:
+#   I int / enum   L int64_t   Q uint64_t / unsigned long long   Z size_t   F float   D double   P any pointer (incl. tg_stream_t)
+#   S const char*.  lib() turns this into ctypes argtypes / restype, so a call with the wrong number or kind of arguments raises
+# instead of shifting every later argument by one slot; tests/test_host_abi.py re-derives the table from the header.
+SIGNATURES = {
+    "tg_status_string": ("S", "I"),
+    "tg_last_error": ("S", ""),
+    "tg_version": ("I", ""),
+    "tg_launch_count": ("Q", ""),
+    "tg_probe_gather": ("I", "PIIIPPPP"),
+    "tg_supported": ("I", "III"),
+    "tg_block_workspace_bytes": ("I", "LLIP"),
+    "tg_block_build": ("I", "LLPPPPIPPPPPPPPPPPZPP"),
+    "tg_sched_workspace_bytes": ("I", "LLLP"),
+    "tg_block_from_csr": ("I", "LLLPPPPPPZPP"),
+    "tg_block_destroy": ("I", "P"),
+    "tg_block_info": ("I", "PPPPP"),
+    "tg_block_sched_info": ("I", "PP"),
+    "tg_block_build_retries": ("Q", ""),
+    "tg_tcsr_workspace_bytes": ("I", "LLP"),
+    "tg_tcsr_build": ("I", "LLPPPPPPPPZP"),
+    "tg_sample_workspace_bytes": ("I", "LP"),
+    "tg_sample_neighbors": ("I", "IIQLPPLPPPPPPPPPPZP"),
+    "tg_sddmm": ("I", "PIIIPPFPP"),
+    "tg_edge_softmax_fwd": ("I", "PIPPP"),
+    "tg_edge_softmax_bwd": ("I", "PIPPPP"),
+    "tg_aggregate_fwd": ("I", "PIIIPPPPZP"),
+    "tg_aggregate_bwd": ("I", "PIIIPPPPPPZP"),
+    "tg_block_coo_dst": ("I", "PPP"),
+    "tg_aggregate_coo": ("I", "PIIIIPPPP"),
+    "tg_attn_workspace_bytes": ("I", "PIIIPP"),
+    "tg_attn_fused_fwd": ("I", "PIIIPPPFPPPPZP"),
+    "tg_attn_fused_bwd": ("I", "PIIIPPPPPPPFPPPPZP"),
+    "tg_attn_fused_bwd_dst": ("I", "PIIIPPPPPPPFPPZP"),
+    "tg_attn_fused_bwd_src": ("I", "PIIIPPPPFPPPZP"),
+    "tg_attn_edge_fused_fwd": ("I", "PIIIPPPPPFFPPPZP"),
+    "tg_attn_edge_fused_bwd": ("I", "PIIIPPPPPPPPFFPPPPPPZP"),
+    "tg_cache_greedy_select": ("I", "DLPPPPLLPPPP"),
+    "tg_cache_lookup_workspace_bytes": ("I", "LP"),
+    "tg_cache_lookup": ("I", "LPPPPPPZP"),
+    "tg_cache_lookup_static": ("I", "LPPPPPP"),
+    "tg_feature_reconstruct": ("I", "LLPPPPPP"),
+}
+EXPORTS = list(SIGNATURES)
+_CTYPE = {"I": C.c_int, "L": C.c_int64, "Q": C.c_uint64, "Z": C.c_size_t, "F": C.c_float, "D": C.c_double, "P": C.c_void_p, "S": C.c_char_p}
 
 
 class FastTGError(RuntimeError):
@@ -45,11 +79,10 @@ def lib() -> C.CDLL:
         if not os.path.exists(_LIB_PATH):
             raise FileNotFoundError(f"{_LIB_PATH} not found: run `python -m paper_2607_05095_b200.build` (no CPU fallback exists)")
         L = C.CDLL(_LIB_PATH)
-        L.tg_status_string.restype = C.c_char_p
-        L.tg_last_error.restype = C.c_char_p
-        L.tg_launch_count.restype = C.c_ulonglong
-        for name in EXPORTS:
-            getattr(L, name)  # fail loudly on a missing symbol
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(L, name)  # fail loudly on a missing symbol
+            fn.restype = _CTYPE[res]
+            fn.argtypes = [_CTYPE[a] for a in args]
         _lib = L
     return _lib
 
@@ -57,6 +90,11 @@ def lib() -> C.CDLL:
 def launch_count() -> int:
     """tg_launch_count: kernels launched by the library in this process so far."""
     return int(lib().tg_launch_count())
+
+
+def block_build_retries() -> int:
+    """tg_block_build_retries: builds repeated in this process because the speculation was too optimistic."""
+    return int(lib().tg_block_build_retries())
 
 
 def probe_gather(table_rows: int, gathers_per_group: int = 4096, iters: int = 5) -> float:
@@ -142,6 +180,13 @@ class Block:
         _check(lib().tg_block_info(self.handle, C.byref(R), C.byref(E), C.byref(U), stats), "tg_block_info")
         keys = ["dst_group_small", "dst_group_big", "dst_warp_items", "dst_slots", "src_group_small", "src_group_big", "src_warp_items", "src_slots"]
         return {"R": R.value, "E": E.value, "U": U.value, **{k: int(v) for k, v in zip(keys, stats)}}
+
+    def sched_info(self):
+        """tg_block_sched_info: group-tier limit, warp-item chunk, hub count and largest degree of both sides."""
+        out = (C.c_int64 * 8)()
+        _check(lib().tg_block_sched_info(self.handle, out), "tg_block_sched_info")
+        keys = ["group_max", "chunk", "hubs", "max_deg"]
+        return {side + "_" + k: int(out[4 * i + j]) for i, side in enumerate(("dst", "src")) for j, k in enumerate(keys)}
 
     def attn_workspace(self, H: int, D: int, dtype: torch.dtype):
         """(forward, backward) workspaces of this block, cached per (H, D, dtype).  They are shared by every call on the

@@ -14,6 +14,7 @@
 //   4. one D2H of {flags, U, both schedules' totals}, one cudaStreamSynchronize
 // What the host cannot know before step 4 (is the input sorted? how many bits do the ids need?) is SPECULATED from the
 // previous call of this thread and verified in step 4; a wrong guess re-runs the build once with the measured values.
+#include <atomic>
 #include "dispatch.cuh"
 #include "scan.cuh"
 #include "radix_sort.cuh"
@@ -175,6 +176,7 @@ struct BuildFlags {
     int pad;
     int dst_tot[TG_SK + 1];   // schedule totals of the destination side (+ max_deg)
     int src_tot[TG_SK + 1];   // ... of the source side
+    int long_gap;     // sorted input with a run of >= TG_FILL_CAP empty rows: indptr comes from tg_fill_indptr_by_search
 };
 
 // sort key of a neighbour id: 32-bit when all ids fit [0, 2^32), else 64-bit with the sign bit flipped (signed order)
@@ -211,7 +213,8 @@ __global__ void k_scan_lists(int64_t R, int64_t E, const int32_t* __restrict__ r
         }
         if (SORTED) {   // garbage in, nothing out: an out-of-range or unsorted input writes no indptr entry out of bounds
             const int64_t lo = max(prev + 1, (int64_t)0), hi = min(cur, R);
-            for (int64_t v = lo; v <= hi; ++v) indptr[v] = (int32_t)e;
+            if (hi - lo >= TG_FILL_CAP) f->long_gap = 1;   // a long run of empty rows: left to the search kernel (all rows)
+            else for (int64_t v = lo; v <= hi; ++v) indptr[v] = (int32_t)e;
         }
     }
     bad = __reduce_or_sync(0xffffffffu, bad);
@@ -422,6 +425,8 @@ static tg_status_t build_attempt(const BuildArgs& a, const BuildWs& w, bool assu
         k_scan_lists<K, true><<<grid_for(E + 1), 256, 0, stream>>>(R, E, a.root_idx, a.nbr_node, a.edge_id, a.ts, w.flags, a.indptr, a.perm,
                                                                     a.dedup_mode ? keys_a : nullptr, a.eid_csr, a.ts_csr);
         TG_LAUNCH_CHECK("k_scan_lists");
+        tg_fill_indptr_by_search<int32_t, int32_t><<<grid_for(R + 1), 256, 0, stream>>>(E, R, a.root_idx, a.indptr, &w.flags->long_gap);
+        TG_LAUNCH_CHECK("tg_fill_indptr_by_search");
     } else {
         k_scan_lists<K, false><<<grid_for(E + 1), 256, 0, stream>>>(R, E, a.root_idx, a.nbr_node, a.edge_id, a.ts, w.flags, nullptr, nullptr,
                                                                      nullptr, nullptr, nullptr);
@@ -484,9 +489,33 @@ static tg_status_t build_attempt(const BuildArgs& a, const BuildWs& w, bool assu
     return TG_OK;
 }
 
-// what the previous build of this thread found: the speculation of the next one
-static thread_local int g_hint_bits = 24;
-static thread_local bool g_hint_unsorted = false;
+// What the recent builds of this thread found: the speculation of the next one.  The hint is sticky: it keeps the
+// largest key width seen recently (in whole 8-bit radix passes) and "unsorted" from any recent build, and gives them up
+// only after TG_HINT_PATIENCE consecutive builds that needed less.  A thread that alternates between blocks with
+// different needs (16- and 17-bit node ids, sorted and shuffled lists) then pays one unneeded radix pass, or a sort of
+// sorted input, on the smaller ones instead of building the larger ones twice.  tg_block_build_retries() counts the
+// builds that were repeated because the speculation was too optimistic.
+constexpr int TG_HINT_PATIENCE = 8;
+struct BuildHint {
+    int bits = 24;
+    bool unsorted = false;
+    int narrower_streak = 0, narrower_max = 0;   // consecutive builds that needed fewer passes, and the most they needed
+    int sorted_streak = 0;
+    void observe(int need_bits /* < 0: this build sorted no neighbour keys */, bool was_unsorted) {
+        const int need = need_bits >= 64 ? 64 : (need_bits + 7) / 8 * 8;
+        if (need_bits < 0) {}
+        else if (need >= bits) { bits = need; narrower_streak = 0; narrower_max = 0; }
+        else {
+            narrower_max = need > narrower_max ? need : narrower_max;
+            if (++narrower_streak >= TG_HINT_PATIENCE) { bits = narrower_max; narrower_streak = 0; narrower_max = 0; }
+        }
+        if (was_unsorted) { unsorted = true; sorted_streak = 0; }
+        else if (unsorted && ++sorted_streak >= TG_HINT_PATIENCE) { unsorted = false; sorted_streak = 0; }
+    }
+};
+static thread_local BuildHint g_hint;
+static std::atomic<unsigned long long> g_build_retries{0};
+extern "C" unsigned long long tg_block_build_retries(void) { return g_build_retries.load(std::memory_order_relaxed); }
 
 extern "C" tg_status_t tg_block_build(int64_t R, int64_t E, const int32_t* root_idx, const int64_t* nbr_node,
                                       const int64_t* edge_id, const float* ts, int dedup_mode, int32_t* indptr, int32_t* perm,
@@ -519,8 +548,8 @@ extern "C" tg_status_t tg_block_build(int64_t R, int64_t E, const int32_t* root_
         if (st == TG_OK) st = tg_side_build(&b->dst, R, 0, indptr, w.side_dst, w.side_dst_bytes, stream);   // all rows are degree 0
     } else {
         BuildArgs a{R, E, root_idx, nbr_node, edge_id, ts, dedup_mode, indptr, perm, kv_row, uniq_node, t_indptr, t_edge, t_dst, eid_csr, ts_csr};
-        bool unsorted = g_hint_unsorted;
-        int bits = g_hint_bits;
+        bool unsorted = g_hint.unsorted;
+        int bits = g_hint.bits;
         for (int attempt = 0; attempt < 3; ++attempt) {
             BuildFlags fh;
             st = (bits <= 32) ? build_attempt<uint32_t>(a, w, unsorted, bits, b, &fh, stream)
@@ -530,12 +559,12 @@ extern "C" tg_status_t tg_block_build(int64_t R, int64_t E, const int32_t* root_
             const bool wide = fh.nbr_min < 0 || fh.nbr_max > 0xffffffffLL;
             const int need = wide ? 64 : bits_for((uint64_t)fh.nbr_max);
             const bool ok = (unsorted || !fh.unsorted) && (dedup_mode == 0 || bits >= need);
-            g_hint_unsorted = fh.unsorted != 0;
-            g_hint_bits = need;
+            g_hint.observe(dedup_mode ? need : -1, fh.unsorted != 0);   // identity rows sort no neighbour keys: no evidence on the width
             if (ok) break;
-            // the speculation was wrong: once more with what this pass measured
-            unsorted = fh.unsorted != 0;
-            bits = need;
+            // the speculation was wrong: once more with what this pass measured (never less than was speculated)
+            g_build_retries.fetch_add(1, std::memory_order_relaxed);
+            unsorted = unsorted || fh.unsorted != 0;
+            bits = need > bits ? need : bits;
             if (attempt == 2) { tg_set_error("tg_block_build: speculation did not converge"); st = TG_ERR_INTERNAL; }
         }
     }
@@ -547,6 +576,17 @@ extern "C" tg_status_t tg_block_build(int64_t R, int64_t E, const int32_t* root_
 
 extern "C" tg_status_t tg_block_destroy(tg_block_t* b) {
     delete b;
+    return TG_OK;
+}
+
+extern "C" tg_status_t tg_block_sched_info(const tg_block_t* b, int64_t out[8]) {
+    TG_CHECK_PTR(b);
+    if (!out) TG_FAIL(TG_ERR_INVALID_ARG, "tg_block_sched_info: out is null");
+    const tg_side* sides[2] = {&b->dst, &b->src};
+    for (int i = 0; i < 2; ++i) {
+        out[4 * i + 0] = sides[i]->group_max; out[4 * i + 1] = sides[i]->chunk;
+        out[4 * i + 2] = sides[i]->n_hubs;    out[4 * i + 3] = sides[i]->max_deg;
+    }
     return TG_OK;
 }
 

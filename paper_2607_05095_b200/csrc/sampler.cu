@@ -33,11 +33,13 @@ __global__ void k_tcsr_keys(int64_t M, int64_t n_nodes, const int64_t* __restric
 // sorted keys -> indptr (boundary fill: indptr[x] = first position whose key >= x) and the entry arrays
 __global__ void k_tcsr_emit(int64_t M2b, int64_t n_nodes, const uint32_t* __restrict__ skeys, const int32_t* __restrict__ sent,
                             const int64_t* __restrict__ u, const int64_t* __restrict__ v, const float* __restrict__ t,
-                            int64_t* indptr, int64_t* nbr, int64_t* eid, float* ts) {
+                            int64_t* indptr, int64_t* nbr, int64_t* eid, float* ts, int* long_gap) {
     for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p <= M2b; p += (int64_t)gridDim.x * blockDim.x) {
         const int64_t prev = (p == 0) ? -1 : (int64_t)skeys[p - 1];
         const int64_t cur = (p == M2b) ? n_nodes : (int64_t)skeys[p];
-        for (int64_t x = prev + 1; x <= min(cur, n_nodes); ++x) indptr[x] = p;
+        const int64_t hi = min(cur, n_nodes);
+        if (hi - prev > TG_FILL_CAP) *long_gap = 1;   // a long run of nodes without events: tg_fill_indptr_by_search writes all rows
+        else for (int64_t x = prev + 1; x <= hi; ++x) indptr[x] = p;
         if (p < M2b && cur < n_nodes) {
             const int ent = sent[p];
             const int64_t i = ent >> 1;
@@ -85,13 +87,16 @@ extern "C" tg_status_t tg_tcsr_build(int64_t n_nodes, int64_t M, const int64_t* 
     void* rs = c.take(tg_rs_bytes<uint32_t>(n));
     int* bad = static_cast<int*>(c.take(256));
     if (!c.ok()) TG_FAIL(TG_ERR_WORKSPACE, "T-CSR workspace: need %zu bytes, have %zu", c.off, workspace_bytes);
-    TG_CUDA(cudaMemsetAsync(bad, 0, 4, stream));
+    TG_CUDA(cudaMemsetAsync(bad, 0, 8, stream));   // bad[0]: endpoint out of range; bad[1]: a long run of empty rows
     k_tcsr_keys<<<smp_grid(M), 256, 0, stream>>>(M, n_nodes, u, v, ka, bad);
     TG_LAUNCH_CHECK("k_tcsr_keys");
     uint32_t* kres; int32_t* vres;
     TG_TRY((tg_radix_sort<uint32_t>(n, smp_bits((uint64_t)n_nodes), ka, va, true, kb, vb, &kres, &vres, rs, stream)));
-    k_tcsr_emit<<<smp_grid(n + 1), 256, 0, stream>>>(n, n_nodes, kres, vres, u, v, t, tc_indptr, tc_nbr, tc_eid, tc_ts);
+    k_tcsr_emit<<<smp_grid(n + 1), 256, 0, stream>>>(n, n_nodes, kres, vres, u, v, t, tc_indptr, tc_nbr, tc_eid, tc_ts, bad + 1);
     TG_LAUNCH_CHECK("k_tcsr_emit");
+    // keys equal to n_nodes are the self-loop sentinels: "number of keys below x" for x <= n_nodes never counts them
+    tg_fill_indptr_by_search<uint32_t, int64_t><<<smp_grid(n_nodes + 1), 256, 0, stream>>>(n, n_nodes, kres, tc_indptr, bad + 1);
+    TG_LAUNCH_CHECK("tg_fill_indptr_by_search");
     int hbad = 0;
     TG_CUDA(cudaMemcpyAsync(&hbad, bad, 4, cudaMemcpyDeviceToHost, stream));
     TG_CUDA(cudaStreamSynchronize(stream));

@@ -137,3 +137,26 @@ static tg_status_t tg_scan(int64_t n, In in, Out out, void* tmp, IVec<K>* total_
     }
     return TG_OK;
 }
+
+// ---------------------------------------------------------------------------------------------
+// Boundary fill of a CSR indptr from sorted keys.  The single-pass builders (block.cu k_scan_lists, sampler.cu
+// k_tcsr_emit) let the thread that sees a key boundary write indptr for the rows in between: fine for the few empty
+// rows of a dense batch, a serial loop of up to n_rows stores when one long run of rows is empty (n_rows >> n, or an
+// empty tail).  They therefore fill only gaps shorter than TG_FILL_CAP and raise a flag otherwise; this kernel, launched
+// behind them, returns at once unless the flag is set and then writes every row by binary search:
+// indptr[x] = number of keys below x, x in [0, n_rows].  Unsorted keys give in-range garbage, never a stray write.
+// ---------------------------------------------------------------------------------------------
+constexpr int TG_FILL_CAP = 32;
+template <class KeyT, class PtrT>
+__global__ void __launch_bounds__(256) tg_fill_indptr_by_search(int64_t n, int64_t n_rows, const KeyT* __restrict__ keys,
+                                                                PtrT* __restrict__ indptr, const int* __restrict__ enable) {
+    if (*enable == 0) return;
+    for (int64_t x = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; x <= n_rows; x += (int64_t)gridDim.x * blockDim.x) {
+        int64_t lo = 0, hi = n;   // first position whose key is >= x
+        while (lo < hi) {
+            const int64_t mid = (lo + hi) >> 1;
+            if ((int64_t)keys[mid] < x) lo = mid + 1; else hi = mid;
+        }
+        indptr[x] = (PtrT)lo;
+    }
+}

@@ -1,7 +1,7 @@
 """GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
 same seeded inputs.  Index structures bit-exact; floating point within BASELINE.json's tolerances.
-Sizes are chosen so that every degree tier (small <= 8, warp <= 256, cta chunks of 8192, hub partial
-merge) and a ragged tail are exercised while the oracle still finishes in seconds."""
+Sizes are chosen so that every degree tier (group tier up to 8 / up to the side's group_max edges, warp-tier chunks of
+64..1024 edges, hub rows merged from several chunks) and a ragged tail are exercised while the oracle still finishes in seconds."""
 import math
 
 import numpy as np
@@ -74,17 +74,67 @@ def test_block_build_bit_exact(B, oracle_mod, w, dedup):
         assert got.dtype == ref.dtype and np.array_equal(got, ref), name
     info = gb.info()
     assert info["R"] == w.R and info["E"] == w.E and info["U"] == ob.U
-    deg = np.diff(ob.indptr)
-    # group tier: rows up to 64 edges on a large side; a launch-bound side (< 2^20 edges) sends rows above a build-time
-    # limit (TG_GROUP_MAX_SMALL_N) to the warp tier instead -- the schedule must be consistent with one such limit
-    limits = (64,) if w.E >= (1 << 20) else (16, 32, 64)
-    assert info["dst_group_small"] == int((deg <= 8).sum())
-    lim = [L for L in limits if info["dst_group_big"] == int(((deg > 8) & (deg <= L)).sum())]
-    assert lim, (info, limits)
-    chunk = 64
-    while chunk < 1024 and w.E // chunk > 148 * 16 * 4:
-        chunk *= 2
-    assert any(info["dst_warp_items"] == int(np.ceil(deg[deg > L] / chunk).sum()) for L in lim)
+    # Schedule statistics against the block's own parameters (tg_block_sched_info), exactly, on both sides.  A side with
+    # >= 2^20 edges keeps rows of up to 64 edges in the group tier; a launch-bound side uses the build's smaller limit.
+    sched = gb.sched_info()
+    for side, ptr in (("dst", ob.indptr), ("src", ob.t_indptr[:ob.U + 1])):
+        deg = np.diff(ptr)
+        lim, chunk = sched[side + "_group_max"], sched[side + "_chunk"]
+        assert lim == 64 if w.E >= (1 << 20) else lim in (16, 32), (side, sched)
+        want_chunk = 64
+        while want_chunk < 1024 and w.E // want_chunk > 148 * 16 * 4:
+            want_chunk *= 2
+        assert chunk == want_chunk, (side, sched)
+        big = deg[deg > lim]
+        assert info[side + "_group_small"] == int((deg <= 8).sum()), side
+        assert info[side + "_group_big"] == int(((deg > 8) & (deg <= lim)).sum()), side
+        assert info[side + "_warp_items"] == int(np.ceil(big / chunk).sum()), side
+        assert sched[side + "_hubs"] == int((big > chunk).sum()), side
+        assert info[side + "_slots"] == int(np.ceil(big[big > chunk] / chunk).sum()), side
+        assert sched[side + "_max_deg"] == (int(deg.max()) if deg.size and deg.max() > 8 else 0), side
+
+
+def test_block_build_speculation_is_sticky(B, oracle_mod):
+    """A thread that alternates between blocks with different needs (sorted / shuffled lists, 16- / 17-bit neighbour ids)
+    repeats a build only when the need grows: the hint follows the largest recent need (tg_block_build_retries)."""
+    narrow = W.small_random(21, 300, 9, 200, 2, 4, shuffle=False)           # sorted roots, ids < 2^16
+    wide = W.small_random(22, 300, 9, 200, 2, 4, shuffle=True)
+    wide.nbr_node = wide.nbr_node + (1 << 16)                                # shuffled roots, 17-bit ids: one more radix pass
+    ref = {id(w): _oblock(oracle_mod, w, 1) for w in (narrow, wide)}
+    gpu_block(B, wide, 1)                                                     # whatever the hint was, it now covers `wide`
+    before = B.block_build_retries()
+    for w in (narrow, wide) * 6:
+        gb = gpu_block(B, w, 1)
+        for name in ("indptr", "perm", "kv_row", "uniq_node", "t_indptr", "t_edge", "t_dst"):
+            assert np.array_equal(host(getattr(gb, name)), getattr(ref[id(w)], name)), (w.name, name)
+    assert B.block_build_retries() == before, "alternating builds must not re-run once the hint covers the larger one"
+    for _ in range(10):                                                       # a long run of small builds relaxes the hint ...
+        gpu_block(B, narrow, 1)
+    gpu_block(B, wide, 1)                                                     # ... and the next large one pays one retry
+    assert B.block_build_retries() == before + 1
+
+
+@pytest.mark.parametrize("where", ["tail", "middle", "head", "short_gaps_only"])
+def test_block_build_long_runs_of_empty_rows(B, oracle_mod, where):
+    """Sorted lists with R >> E: a run of empty destinations longer than the in-kernel fill handles (>= 32 rows) is
+    filled by the search kernel; runs just below the limit stay on the single-pass path.  Bit-exact either way."""
+    rng = np.random.default_rng(5)
+    R = 2_000_003
+    if where == "short_gaps_only":
+        R = 40_000
+        roots = np.arange(0, R, 31)                                           # gaps of 30 empty rows, none at the tail beyond 31
+    else:
+        lo = {"tail": 0, "middle": 0, "head": R - 700}[where]
+        roots = np.sort(rng.integers(lo, lo + 700, size=1500))
+        if where == "middle":
+            roots = np.concatenate([roots, [R - 1, R - 1]])
+    E = len(roots)
+    nbr = rng.integers(0, 300, size=E).astype(np.int64)
+    ob = oracle_mod.block_build(R, roots.astype(np.int32), nbr, None, None, 1)
+    gb = B.block_build(R, dev(roots.astype(np.int32)), dev(nbr), None, None, 1)
+    for name in ("indptr", "perm", "kv_row", "uniq_node", "t_indptr", "t_edge", "t_dst"):
+        assert np.array_equal(host(getattr(gb, name)), getattr(ob, name)), (where, name)
+    assert gb.info()["dst_group_small"] == int((np.diff(ob.indptr) <= 8).sum())
 
 
 def test_block_build_negative_ids_and_empty(B, oracle_mod):

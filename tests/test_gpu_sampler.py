@@ -76,6 +76,21 @@ def test_empty_stream(B):
     assert got[0].numel() == 0
 
 
+def test_tcsr_long_runs_of_nodes_without_events(B):
+    """n_nodes >> M: the runs of event-free nodes are longer than the emit kernel fills itself (the search kernel writes
+    tc_indptr then), including a run at the tail and self-loops, whose sentinel entries sort behind every node."""
+    rng = np.random.default_rng(9)
+    n_nodes, M = 1_500_007, 900
+    u = rng.integers(0, 400, size=M)
+    v = rng.integers(700_000, 700_300, size=M)
+    u[::50] = v[::50]                                                        # some self-loops
+    t = np.sort(rng.random(M)).astype(np.float32)
+    o = S.tcsr_build(n_nodes, u, v, t)
+    g = _gpu_tcsr(B, n_nodes, u, v, t)
+    _check_tcsr(g, o)
+    _check_sample(B, g, o, [int(v[-1]), int(u[3]), n_nodes - 1], [M, M, M], 5, "recent")
+
+
 def _stream_case(B, oracle_mod, cid, n_nodes, n_events, k, hop2=False):
     seed = 0
     u, v, t = W._event_stream(seed, cid, n_nodes, n_events)
