@@ -17,7 +17,6 @@ import argparse
 import json
 import math
 import os
-import subprocess
 import sys
 import threading
 import time
@@ -44,7 +43,7 @@ def measured_hbm_gbs():
 
 
 def make_workloads(cfg: int, seed: int, src_nodes: int = 0):
-    from paper_2607_05095_b200 import workloads as W
+    import workloads as W
     if src_nodes > 0:   # diagnostic: config 4's degree structure over `src_nodes` source nodes (16: every gather hits L1)
         assert cfg == 4, "--src-nodes is a config-4 diagnostic"
         w = W.config4(seed, n_src_nodes=src_nodes)
@@ -309,13 +308,30 @@ def run_extras(args, B, blocks, bi_dom, extras, peak):
         B.block_build(w.R, root_d, nbr_d, None, None, w.dedup_mode)
     torch.cuda.synchronize()
     bms = (time.perf_counter() - t0) * 1e3 / 5
+    # the same call with its outputs and workspace pre-allocated (block_build(reuse=...): no torch.empty inside), timed by CUDA
+    # events on the launching stream; the call still ends with its one synchronisation, so host gaps between calls are inside
+    rb = B.block_build(w.R, root_d, nbr_d, None, None, w.dedup_mode)
+    be = [torch.cuda.Event(enable_timing=True) for _ in range(11)]
+    torch.cuda.synchronize()
+    retries0 = B.block_build_retries()
+    be[0].record()
+    for i in range(10):
+        rb = B.block_build(w.R, root_d, nbr_d, None, None, w.dedup_mode, reuse=rb)
+        be[i + 1].record()
+    torch.cuda.synchronize()
+    bms_pre = float(np.median([be[i].elapsed_time(be[i + 1]) for i in range(10)]))
+    assert torch.equal(rb.kv_row, bb["blk"].kv_row) and rb.U == bb["blk"].U
     U_ = bb["blk"].U
     # A0's algorithmic bytes: the sampler lists in (root_idx i32, nbr_node i64), every public index array out once
     bbytes = 12 * w.E + 4 * (w.R + 1) + 4 * w.E + ((4 * w.E + 8 * U_ + 4 * (U_ + 1) + 8 * w.E) if w.dedup_mode else 0)
     extras["block_build_ms"] = bms
     extras["block_build"] = {"ms": bms, "algorithmic_bytes": bbytes, "achieved_gbs": bbytes / (bms * 1e-3) / 1e9,
                              "frac_of_measured_copy": bbytes / (bms * 1e-3) / 1e9 / peak,
-                             "timing": "host wall clock around 5 calls (the call synchronises to return U), output allocation included"}
+                             "timing": "host wall clock around 5 calls (the call synchronises to return U), output allocation included",
+                             "ms_preallocated": bms_pre, "frac_of_measured_copy_preallocated": bbytes / (bms_pre * 1e-3) / 1e9 / peak,
+                             "timing_preallocated": "median of 10 calls with outputs and workspace reused, CUDA events on the launching stream",
+                             "retries_in_timed_calls": B.block_build_retries() - retries0}
+    del rb
     if not args.no_unfused:
         d, o, blk = bb["dev"], bb["out"], bb["blk"]
         s = torch.empty(w.E, w.H, dtype=torch.float32, device="cuda")
@@ -434,7 +450,7 @@ def run_next34(args, B, blocks, bi_dom, extras, peak):
         extras["plain_agg"] = res
         del Yc, Xc, dXs, coo
     if not args.no_sampler:
-        from paper_2607_05095_b200 import workloads as W
+        import workloads as W
         n_nodes, n_events, n_roots, k = 100_000, 5_000_000, 200_000, 10
         u, v, t = W._event_stream(args.seed, 2, n_nodes, n_events)
         ud, vd, td = (torch.from_numpy(np.ascontiguousarray(x)).cuda() for x in (u.astype(np.int64), v.astype(np.int64), t.astype(np.float32)))
@@ -463,7 +479,7 @@ def run_e2e_sampled(args, B, extras):
     K / V row gather (tg_cache_lookup + tg_feature_reconstruct, every row resident) and the fused forward + backward run
     on the device; O, dQ, dK, dV come back.  No sampled list and no feature row crosses PCIe."""
     import torch
-    from paper_2607_05095_b200 import workloads as W
+    import workloads as W
     cid = args.config
     n_nodes, n_events, batch, k, mode = {1: (20_000, 200_000, 600, 10, "recent"), 3: (1_000_000, 50_000_000, 4000, 20, "uniform")}[cid]
     H, D, dt = {1: (2, 50, torch.float32), 3: (4, 32, torch.bfloat16)}[cid]
@@ -512,6 +528,103 @@ def run_e2e_sampled(args, B, extras):
                              "d2h_bytes_per_step": d2h, "resident_bytes": int(Ktab.numel() * Ktab.element_size() * 2 + g.nbr.numel() * 20),
                              "sampling": f"{mode}, k = {k}, on the device", "steps": n,
                              "note": "host sends roots + Q + dO, receives O, dQ, dK, dV; T-CSR and node-level K / V tables resident in HBM; synchronous steps (no overlap)"}
+
+
+def step_spread(per_step_ms, how):
+    """median / min / p10 / p90 of single-step device times ('report median, min, p10/p90')."""
+    a = np.sort(np.asarray(per_step_ms, dtype=np.float64))
+    if a.size == 0:
+        return None
+    return {"median": float(np.median(a)), "min": float(a[0]), "p10": float(np.percentile(a, 10)), "p90": float(np.percentile(a, 90)),
+            "max": float(a[-1]), "n": int(a.size), "rank": 0, "how": how}
+
+
+def relaunch_under_torchrun(n_gpus: int) -> int:
+    """`python bench.py --gpus N` with N > 1 and no rendezvous in the environment: start the N ranks ourselves, exactly as the
+    driver's launch line does (one process per GPU, 127.0.0.1 rendezvous), and pass the ranks' output through.  NCCL's
+    communicator log is switched on (unless the caller set NCCL_DEBUG) so that the number of ranks in the barrier / all-reduce
+    communicator can be read off; its lines go to stderr, stdout stays the one JSON line of rank 0."""
+    import socket
+    import subprocess
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = so.getsockname()[1]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n_gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+    p = subprocess.Popen(cmd, env=env, stdout=subprocess.PIPE, text=True)
+    for ln in p.stdout:
+        (sys.stderr if " NCCL " in ln else sys.stdout).write(ln)
+    return p.wait()
+
+
+def other_configs_extras(args, B, peak):
+    """Configs 1-3 (launch-bound: the working set fits in L2) in the default line: one CUDA-graph replay of the fused
+    fwd + bwd step per config, warm (back-to-back replays) and cold (256 MB L2 flush before every replay, outside the events).
+    Not the headline: the driver never runs these configs by themselves."""
+    import torch
+    TDT = {"f32": torch.float32, "bf16": torch.bfloat16}
+    out = {}
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    for c in (1, 2, 3):
+        if c == args.config:
+            continue
+        ws = make_workloads(c, args.seed)
+        items, comp_bytes = [], 0
+        for w in ws:
+            dt = TDT[w.dtype]
+            blk = B.block_build(w.R, torch.from_numpy(w.root_idx).cuda(), torch.from_numpy(w.nbr_node).cuda(), None, None, w.dedup_mode)
+            q, k, v, do = (torch.from_numpy(x).to(dt).cuda() for x in w.features(blk.U))
+            o = dict(O=torch.empty_like(q), lse=torch.empty(w.R, w.H, dtype=torch.float32, device="cuda"), dQ=torch.empty_like(q),
+                     dK=torch.empty_like(k), dV=torch.empty_like(v))
+            items.append((w, blk, q, k, v, do, o))
+            comp_bytes += sum(call_bytes(w.R, w.E, blk.U, w.H, w.D, 2 if w.dtype == "bf16" else 4, w.dedup_mode).values())
+
+        def step():
+            for w, blk, q, k, v, do, o in items:
+                B.attn_fused_fwd(blk, q, k, v, w.scale, out=(o["O"], o["lse"]))
+                B.attn_fused_bwd_dst(blk, q, k, v, o["O"], o["lse"], do, w.scale, o["dQ"])
+                B.attn_fused_bwd_src(blk, q, k, v, do, w.scale, o["dK"], o["dV"])
+
+        for _ in range(3):
+            step()
+        g, cs = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+        cs.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(cs):
+            step()
+        torch.cuda.current_stream().wait_stream(cs)
+        with torch.cuda.graph(g, stream=cs):
+            step()
+        n = 50
+        for _ in range(5):
+            g.replay()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(n + 1)]
+        torch.cuda.synchronize()
+        ev[0].record()
+        for i in range(n):
+            g.replay()
+            ev[i + 1].record()
+        torch.cuda.synchronize()
+        warm = [ev[i].elapsed_time(ev[i + 1]) for i in range(n)]
+        ce = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(20)]
+        for i, (a, b_) in enumerate(ce):
+            flush.fill_(i & 255)
+            a.record()
+            g.replay()
+            b_.record()
+        torch.cuda.synchronize()
+        cold = float(np.median([a.elapsed_time(b_) for a, b_ in ce]))
+        E = sum(it[0].E for it in items)
+        wm = float(np.median(warm))
+        out[f"config{c}"] = {"workload": "+".join(it[0].name for it in items), "E": E, "graph_ms_per_step": wm, "min_ms": float(min(warm)),
+                             "edges_per_s": E / (wm * 1e-3), "cold_l2_ms_per_step": cold, "compulsory_bytes": comp_bytes,
+                             "cold_frac_of_measured_copy": comp_bytes / (cold * 1e-3) / 1e9 / peak,
+                             "byte_time_us_at_measured_copy": comp_bytes / (peak * 1e9) * 1e6}
+        del g, items
+    del flush
+    return out
 
 
 def run_ours(args):
@@ -606,6 +719,23 @@ def run_ours(args):
         graph_ms = timed(lambda i: g.replay(), args.steps, sampler)
         total_ms, launch_mode = graph_ms, "cuda_graph_replay (the step's C-ABI calls captured once; tg_* calls are capturable)"
     clocks = sampler.stop() if rank == 0 else None
+    # spread of single steps (SURVEY.md §8(d) timing protocol), this rank: one event pair per step.  Eager: the events already
+    # recorded inside the headline region (first call's start -> last call's end, so launch gaps BETWEEN steps are not in it);
+    # graph: a separate pass of the same length with an event between replays (the headline region has none).
+    if use_graph:
+        se = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+        barrier()
+        se[0].record()
+        for i in range(args.steps):
+            g.replay()
+            se[i + 1].record()
+        barrier()
+        per_step = [se[i].elapsed_time(se[i + 1]) for i in range(args.steps)]
+        spread_how = "separate pass: one event between consecutive graph replays"
+    else:
+        per_step = [evs[i][0][0].elapsed_time(evs[i][-1][3]) for i in range(args.steps)]
+        spread_how = "events of the headline region: first call's start to last call's end of each step"
+    step_ms = step_spread(per_step, spread_how)
     E_local = sum(b["w"].E for b in blocks)
     total_ms, E_all = reduce_over_ranks(total_ms, E_local, world, "cuda")
     ms_per_step = total_ms / args.steps
@@ -760,14 +890,16 @@ def run_ours(args):
         run_next34(args, B, blocks, bi_dom, extras, peak)
     if args.e2e_sampled and args.config in (1, 3):
         run_e2e_sampled(args, B, extras)
+    if not args.no_other_configs and not args.no_unfused:
+        extras["other_configs"] = other_configs_extras(args, B, peak)
     extras["kernel_ms"] = kms
-    extras["schedule"] = blocks[bi_dom]["info"]
+    extras["schedule"] = {**blocks[bi_dom]["info"], **blocks[bi_dom]["blk"].sched_info()}
 
     cpu = None if args.no_cpu else oracle_cpu_baseline([bb["w"] for bb in blocks], args.cpu_full_edges, args.cpu_edges)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warm,
-        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms_per_step, "step_ms": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16" if w.dtype == "bf16" else "f32", "data": "synthetic", "config": cfg,
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(round(launches_per_step * args.steps)), "roofline": roofline, "hbm": hbm,
         "cpu_baseline": cpu, "extras": extras,
@@ -797,6 +929,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-unfused", action="store_true", help="skip the extras: unfused chain, edge term, SlimCache, plain AGG, sampler")
     ap.add_argument("--no-sampler", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip extras.other_configs (configs 1-3, graph-replayed; ~45 s of host-side input generation)")
     ap.add_argument("--e2e-sampled", action="store_true", help="configs 1, 3: extras.e2e_sampled = the step with the sampler and the feature rows on the device")
     ap.add_argument("--side-copy", action="store_true", help="bf16 storage: the forward writes a float32 side copy of O, the backward takes delta from it")
     args = ap.parse_args()
@@ -805,7 +938,16 @@ def main():
         rows = {"l1_64rows_16KB": 64, "l1_512rows_128KB": 512, "l2_65536rows_16MB": 65536, "dram_8Mrows_2GB": 8 << 20}
         print(json.dumps({"probe": "256-byte row gathers, 8 lanes x 2 LDG.128 per row", "unit": "GB/s",
                           **{k: round(B.probe_gather(v), 1) for k, v in rows.items()}}))
+        for stages in (2, 4, 8):
+            res = {k: B.probe_gather_bulk(v, stages) for k, v in rows.items()}
+            print(json.dumps({"probe": f"the same gathers as cp.async.bulk (256 bytes per row, one elected lane per group) into a ring of {stages} "
+                                       "shared-memory stages per warp, mbarrier completion, 2 LDS.128 per lane",
+                              "unit": "GB/s", "ctas_per_sm": next(iter(res.values()))[1], **{k: round(v[0], 1) for k, v in res.items()}}))
         return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        raise SystemExit(relaunch_under_torchrun(args.gpus))
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:   # one line per rank, before any heavy import: who was started
+        print(f"[bench.py] rank {os.environ.get('RANK', '?')}/{os.environ['WORLD_SIZE']} started", file=sys.stderr, flush=True)
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -72,13 +72,6 @@ TG_API int tg_version(void);
 /* Number of kernels this library has launched in the process so far (all threads, all streams):
  * the difference across a timed region is the library's launch count for it. */
 TG_API unsigned long long tg_launch_count(void);
-/* Diagnostic, not part of the hot path: times `iters` launches of a pure row-gather kernel (every group of 8
- * lanes reads 256-byte rows at pseudo-random indices of `table` [table_rows, 256 bytes] DEVICE, the access shape
- * of the attention kernels) and returns the milliseconds and the bytes gathered (HOST outputs).  With a small
- * table every access hits L1: bytes / ms is the L1 gather roof quoted in DESIGN.md section 7.  `sink`: 4 DEVICE
- * bytes.  Synchronises the stream. */
-TG_API tg_status_t tg_probe_gather(const void* table, int table_rows, int gathers_per_group, int iters, void* sink,
-                                   tg_stream_t stream, float* ms /*HOST*/, double* bytes /*HOST*/);
 /* 1 if (H, D, dtype) has a compiled kernel path, else 0. */
 TG_API int tg_supported(int H, int D, tg_dtype_t dtype);
 

@@ -14,7 +14,7 @@ driven by a counter-based generator (SplitMix64 outputs indexed by (seed, root, 
 
 Plain NumPy / pure-Python loops over roots, no blocking, no vectorised tricks: written to be checked by eye.
 Pins (tests/test_oracle_sampler.py): brute force over the raw event list on tiny streams; the bench generator's own
-dictionary-based sampler (paper_2607_05095_b200/workloads._sample_block) on config 1; SplitMix64's published test
+dictionary-based sampler (workloads._sample_block) on config 1; SplitMix64's published test
 vector; Floyd's algorithm against exhaustive subset frequencies; validity properties of every draw.
 """
 from __future__ import annotations

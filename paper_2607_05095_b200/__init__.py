@@ -5,4 +5,4 @@ The product is the C-ABI shared library ``libfasttg.so`` (hand-written sm_100a C
 Importing this package does not load the library; ``binding.lib()`` does and fails loudly if it
 is missing.
 """
-__all__ = ["binding", "workloads", "build"]
+__all__ = ["binding", "build"]

@@ -19,7 +19,7 @@ _lib = None
 TG_F32, TG_BF16 = 0, 1
 _DTYPES = {torch.float32: TG_F32, torch.bfloat16: TG_BF16}
 
-# Signature of every export of include/fasttg.h: name -> (result, arguments), one letter per C type:
+# Signature of every export of include/fasttg.h and include/fasttg_diag.h: name -> (result, arguments), one letter per C type:
 #   I int / enum   L int64_t   Q uint64_t / unsigned long long   Z size_t   F float   D double   P any pointer (incl. tg_stream_t)
 #   S const char*.  lib() turns this into ctypes argtypes / restype, so a call with the wrong number or kind of arguments raises
 # instead of shifting every later argument by one slot; tests/test_host_abi.py re-derives the table from the header.
@@ -29,6 +29,7 @@ SIGNATURES = {
     "tg_version": ("I", ""),
     "tg_launch_count": ("Q", ""),
     "tg_probe_gather": ("I", "PIIIPPPP"),
+    "tg_probe_gather_bulk": ("I", "PIIIIPPPPP"),
     "tg_supported": ("I", "III"),
     "tg_block_workspace_bytes": ("I", "LLIP"),
     "tg_block_build": ("I", "LLPPPPIPPPPPPPPPPPZPP"),
@@ -107,6 +108,16 @@ def probe_gather(table_rows: int, gathers_per_group: int = 4096, iters: int = 5)
     return nbytes.value / (ms.value * 1e-3) / 1e9
 
 
+def probe_gather_bulk(table_rows: int, stages: int = 4, gathers_per_group: int = 4096, iters: int = 5):
+    """tg_probe_gather_bulk: (GB/s, resident CTAs per SM) of the same gathers issued as cp.async.bulk into a shared-memory ring."""
+    table = torch.randint(0, 2 ** 31 - 1, (table_rows, 64), dtype=torch.int32, device="cuda")
+    sink = torch.zeros(2, dtype=torch.int32, device="cuda")
+    ms, nbytes, occ = C.c_float(0), C.c_double(0), C.c_int(0)
+    _check(lib().tg_probe_gather_bulk(_ptr(table), C.c_int(table_rows), C.c_int(gathers_per_group), C.c_int(stages), C.c_int(iters),
+                                      _ptr(sink), _stream(), C.byref(ms), C.byref(nbytes), C.byref(occ)), "tg_probe_gather_bulk")
+    return nbytes.value / (ms.value * 1e-3) / 1e9, occ.value
+
+
 def _check(st: int, where: str):
     if st != 0:
         L = lib()
@@ -164,13 +175,19 @@ class Block:
         self.indptr = self.perm = self.kv_row = self.uniq_node = None
         self.t_indptr = self.t_edge = self.t_dst = self.eid_csr = self.ts_csr = None
         self._ws = None
+        self._full = None      # block_build: the full-capacity output arrays and the workspace (block_build(reuse=...))
         self._attn_ws = {}
+
+    def destroy(self):
+        """tg_block_destroy; the Block must not be used afterwards (its arrays may be handed to another build)."""
+        if self.handle and _lib is not None:
+            _lib.tg_block_destroy(self.handle)
+        self.handle = C.c_void_p(0)
+        self._full = None
 
     def __del__(self):
         try:
-            if self.handle and _lib is not None:
-                _lib.tg_block_destroy(self.handle)
-                self.handle = C.c_void_p(0)
+            self.destroy()
         except Exception:
             pass
 
@@ -203,8 +220,10 @@ class Block:
 
 
 def block_build(R: int, root_idx: torch.Tensor, nbr_node: torch.Tensor, edge_id: torch.Tensor | None = None,
-                ts: torch.Tensor | None = None, dedup_mode: int = 1) -> Block:
-    """tg_block_build.  root_idx int32 [E], nbr_node int64 [E], edge_id int64 [E] | None, ts float32 [E] | None (CUDA)."""
+                ts: torch.Tensor | None = None, dedup_mode: int = 1, reuse: Block | None = None) -> Block:
+    """tg_block_build.  root_idx int32 [E], nbr_node int64 [E], edge_id int64 [E] | None, ts float32 [E] | None (CUDA).
+    reuse: a Block of the same (R, E, dedup_mode, pass-through arrays) whose output arrays and workspace are taken over
+    instead of allocating new ones (a training loop with a fixed batch shape); that Block is destroyed by the call."""
     L = lib()
     dev = root_idx.device
     if not root_idx.is_cuda:
@@ -220,18 +239,24 @@ def block_build(R: int, root_idx: torch.Tensor, nbr_node: torch.Tensor, edge_id:
         ts = ts.contiguous()
     b = Block()
     i32 = dict(dtype=torch.int32, device=dev)
-    b.indptr = torch.empty(R + 1, **i32)
-    b.perm = torch.empty(E, **i32)
-    b.kv_row = torch.empty(E, **i32)
-    b.uniq_node = torch.empty(max(E, 1), dtype=torch.int64, device=dev)
-    b.t_indptr = torch.empty(E + 1, **i32)
-    b.t_edge = torch.empty(E, **i32)
-    b.t_dst = torch.empty(E, **i32)
-    b.eid_csr = None if edge_id is None else torch.empty(E, dtype=torch.int64, device=dev)
-    b.ts_csr = None if ts is None else torch.empty(E, dtype=torch.float32, device=dev)
     nbytes = C.c_size_t()
     _check(L.tg_block_workspace_bytes(C.c_int64(R), C.c_int64(E), C.c_int(dedup_mode), C.byref(nbytes)), "tg_block_workspace_bytes")
-    b._ws = torch.empty(nbytes.value, dtype=torch.uint8, device=dev)
+    key = (R, E, dedup_mode, edge_id is not None, ts is not None, dev, nbytes.value)
+    if reuse is not None:
+        if reuse._full is None or reuse._full["key"] != key:
+            raise ValueError("block_build(reuse=...): the Block to reuse was built for another shape")
+        full = reuse._full
+        reuse.destroy()
+    else:
+        full = dict(key=key, indptr=torch.empty(R + 1, **i32), perm=torch.empty(E, **i32), kv_row=torch.empty(E, **i32),
+                    uniq_node=torch.empty(max(E, 1), dtype=torch.int64, device=dev), t_indptr=torch.empty(E + 1, **i32),
+                    t_edge=torch.empty(E, **i32), t_dst=torch.empty(E, **i32),
+                    eid_csr=None if edge_id is None else torch.empty(E, dtype=torch.int64, device=dev),
+                    ts_csr=None if ts is None else torch.empty(E, dtype=torch.float32, device=dev),
+                    ws=torch.empty(nbytes.value, dtype=torch.uint8, device=dev))
+    b._full = full
+    b.indptr, b.perm, b.kv_row, b.uniq_node, b.t_indptr = full["indptr"], full["perm"], full["kv_row"], full["uniq_node"], full["t_indptr"]
+    b.t_edge, b.t_dst, b.eid_csr, b.ts_csr, b._ws = full["t_edge"], full["t_dst"], full["eid_csr"], full["ts_csr"], full["ws"]
     U = C.c_int64()
     _check(L.tg_block_build(C.c_int64(R), C.c_int64(E), _ptr(root_idx), _ptr(nbr_node), _ptr(edge_id), _ptr(ts),
                             C.c_int(dedup_mode), _ptr(b.indptr), _ptr(b.perm), _ptr(b.kv_row), _ptr(b.uniq_node),

@@ -19,14 +19,14 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libfasttg.so")
-SOURCES = ["api.cu", "block.cu", "fused_fwd.cu", "fused_bwd.cu", "fused_edge.cu", "unfused.cu", "softmax.cu", "cache.cu", "sampler.cu"]
+SOURCES = ["api.cu", "block.cu", "fused_fwd.cu", "fused_bwd.cu", "fused_edge.cu", "unfused.cu", "softmax.cu", "cache.cu", "sampler.cu", "probe_bulk.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC,-fvisibility=hidden", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
 # No --use_fast_math: measured in round 2, it changed neither the errors nor the times; the only approximate
 # instruction on the path is the explicit ex2.approx of the softmax.  TG_FAST_MATH=1 re-enables it for comparison.
 if os.environ.get("TG_FAST_MATH", "0") == "1":
     NVCC_FLAGS.insert(5, "--use_fast_math")
-# tuning knobs (e.g. TG_NVCC_EXTRA="-DTG_FWD_POLICY=1,3,1,4"); part of the build stamp
+# extra nvcc flags for experiments (e.g. TG_NVCC_EXTRA="-DTG_CHUNK_MAX_EDGES=512"); part of the build stamp
 NVCC_FLAGS += os.environ.get("TG_NVCC_EXTRA", "").split()
 
 
@@ -46,7 +46,8 @@ def _stamp() -> str:
         if os.path.isfile(p) and n.endswith((".cu", ".cuh", ".h")):
             h.update(n.encode())
             h.update(open(p, "rb").read())
-    h.update(open(os.path.join(ROOT, "include", "fasttg.h"), "rb").read())
+    for n in sorted(os.listdir(os.path.join(ROOT, "include"))):
+        h.update(open(os.path.join(ROOT, "include", n), "rb").read())
     return h.hexdigest()
 
 

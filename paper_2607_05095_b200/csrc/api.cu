@@ -4,6 +4,7 @@
 #include <atomic>
 
 #include "dispatch.cuh"
+#include "fasttg_diag.h"
 
 static thread_local char g_err[512] = "";
 

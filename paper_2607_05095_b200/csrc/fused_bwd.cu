@@ -2,93 +2,24 @@
 // Pass 1, destination-major: delta, dQ (and the {lse2, delta} table).  Pass 2, source-major over the
 // transposed CSR: dK, dV by gather -- no float atomics, run-to-run bitwise reproducible.
 #include "dispatch.cuh"
-#include "ops_mma.cuh"
+#include "ops.cuh"
 
-// launch policy {edges per trip, min CTAs per SM} for the pipelined and the plain kernel variants
-#ifndef TG_BWD1_U
-#define TG_BWD1_U 1
-#endif
-#ifndef TG_BWD1_CTAS
-#define TG_BWD1_CTAS 2
-#endif
-#ifndef TG_BWD1_UP
-#define TG_BWD1_UP 1
-#endif
-#ifndef TG_BWD1_CTASP
-#define TG_BWD1_CTASP 3
-#endif
-#ifndef TG_BWD1_UW
-#define TG_BWD1_UW TG_BWD1_U
-#endif
-#ifndef TG_BWD1_WARPSW
-#define TG_BWD1_WARPSW (8 * TG_BWD1_CTAS)
-#endif
-#ifndef TG_BWD1_WPIPE
-#define TG_BWD1_WPIPE true
-#endif
-#define TG_BWD1_POLICY TG_BWD1_U, TG_BWD1_CTAS, TG_BWD1_UP, TG_BWD1_CTASP, TG_BWD1_UW, TG_BWD1_WARPSW, TG_BWD1_WPIPE
-#ifndef TG_BWD2_U
-#define TG_BWD2_U 1
-#endif
-#ifndef TG_BWD2_CTAS
-#define TG_BWD2_CTAS 2
-#endif
-#ifndef TG_BWD2_UP
-#define TG_BWD2_UP 1
-#endif
-#ifndef TG_BWD2_CTASP
-#define TG_BWD2_CTASP 3
-#endif
-#ifndef TG_BWD2_UW
-#define TG_BWD2_UW TG_BWD2_U
-#endif
-#ifndef TG_BWD2_WARPSW
-#define TG_BWD2_WARPSW (8 * TG_BWD2_CTAS)
-#endif
-#ifndef TG_BWD2_WPIPE
-#define TG_BWD2_WPIPE true
-#endif
-#define TG_BWD2_POLICY TG_BWD2_U, TG_BWD2_CTAS, TG_BWD2_UP, TG_BWD2_CTASP, TG_BWD2_UW, TG_BWD2_WARPSW, TG_BWD2_WPIPE
-
-// 1: bf16 rows of 256 bytes with D in {16, 32}: the warp tier takes its dot products from HMMA (ops_mma.cuh); 0 (default): FHFMA.
-// Measured on config 4 (profiles/r02_hmma_probe.md): bwd_dst 0.472 -> 0.529 ms, bwd_src 0.557 -> 0.633 ms.
-#ifndef TG_BWD1_MMA
-#define TG_BWD1_MMA 0
-#endif
-#ifndef TG_BWD2_MMA
-#define TG_BWD2_MMA 0
-#endif
-
-// words of a gathered 256-byte bf16 row per lane: 8 = LPR 8 (two vectors per lane), 4 = LPR 16 (one vector per lane: half the
-// buffer / accumulator registers per thread, the same instructions per edge, 24 instead of 16 resident warps).  Measured on config 4
-// (profiles/r01_other_configs_and_probes.md, round-2 additions): forward 0.367 -> 0.352 ms, destination-major backward 0.475 -> 0.450 ms,
-// source-major backward 0.539 -> 0.592 ms -- so the first two use LPR 16, the source-major pass stays at LPR 8.
-#ifndef TG_BWD1_MAXW
-#define TG_BWD1_MAXW 4
-#endif
-#ifndef TG_BWD1_WARPSW16
-#define TG_BWD1_WARPSW16 24
-#endif
-#ifndef TG_BWD2_WARPSW16
-#define TG_BWD2_WARPSW16 24
-#endif
-// fp32 rows of 512 bytes: 16 = the wide single-buffered layout (LPR 8), 8 = LPR 16, 4 = LPR 32, both pipelined.  Measured on config 5:
-// destination-major 6.92 (wide) / 7.69 (LPR 16) / 6.43 ms (LPR 32); source-major 6.20 (wide) / 8.06 / 7.90 ms
-#ifndef TG_BWD1_MAXW_F32
-#define TG_BWD1_MAXW_F32 4
-#endif
-#ifndef TG_BWD2_MAXW_F32
-#define TG_BWD2_MAXW_F32 16
-#endif
-#ifndef TG_BWD1_GROUP_RELAYOUT
-#define TG_BWD1_GROUP_RELAYOUT 1   // 1: the group tiers use the warp tier's layout too
-#endif
-#ifndef TG_BWD2_GROUP_RELAYOUT
-#define TG_BWD2_GROUP_RELAYOUT 0
-#endif
-#ifndef TG_BWD2_MAXW
-#define TG_BWD2_MAXW 8
-#endif
+// Launch policies (TierPolicy<U pipelined, min CTAs/SM pipelined, U plain, min CTAs/SM plain, U warp tier, resident warps/SM of
+// the warp tier, warp tier pipelined>): one edge per trip in both passes.  The values are the round-2 sweep's winners on
+// configs 4 / 5; the alternatives (U = 2, other occupancy caps, source-major loop variants, HMMA dot products) are recorded
+// in profiles/r01_other_configs_and_probes.md and profiles/r02_hmma_probe.md and are no longer in the tree.
+using BwdPolicy = TierPolicy<1, 2, 1, 3, 1, 16, true>;
+using BwdPolicyNarrow = TierPolicy<1, 2, 1, 3, 1, 24, true>;    // one vector per lane: 24 resident warps per SM
+using BwdPolicyWide = TierPolicy<1, 2, 1, 2, 1, 16, false>;     // fp32 rows at 16 words per lane: single-buffered loops
+// Words of a gathered row per lane.  bf16 rows of 256 bytes: 8 = LPR 8 (two vectors per lane), 4 = LPR 16 (one vector per lane:
+// half the buffer / accumulator registers, the same instructions per edge, 24 instead of 16 resident warps).  Measured on
+// config 4: destination-major 0.475 -> 0.450 ms at LPR 16, source-major 0.539 -> 0.592 ms -- so pass 1 uses LPR 16 (group
+// tiers included) and pass 2 stays at LPR 8 with its group tiers in the default layout.  fp32 rows of 512 bytes: 16 = the wide
+// single-buffered layout (LPR 8), 8 = LPR 16, 4 = LPR 32.  Measured on config 5: destination-major 6.92 / 7.69 / 6.43 ms,
+// source-major 6.20 / 8.06 / 7.90 ms.
+constexpr int TG_BWD1_MAXW_BF16_256 = 4, TG_BWD2_MAXW_BF16_256 = 8;
+constexpr int TG_BWD1_MAXW_F32_512 = 4, TG_BWD2_MAXW_F32_512 = 16;
+constexpr bool TG_BWD1_GROUP_RELAYOUT = true, TG_BWD2_GROUP_RELAYOUT = false;
 
 struct BwdArgs {
     const tg_block* b;
@@ -121,14 +52,14 @@ struct BwdFn {
         constexpr bool F512 = !Tr::BF16 && Tr::F * Tr::EB == 512;
         constexpr bool B256 = Tr::BF16 && Tr::F * Tr::EB == 256;
         if (which & 1) {
-            constexpr bool WIDE = !Tr::BF16 && Tr::F * Tr::EB >= 512 && !(F512 && TG_BWD1_MAXW_F32 != 16);
-            using TrW = typename std::conditional<WIDE, RowTraits<T, Tr::H, Tr::D, 16>, typename tg_relayout<Tr, B256 ? TG_BWD1_MAXW : F512 ? TG_BWD1_MAXW_F32 : 8>::type>::type;
-            using TrG = typename std::conditional<WIDE || TG_BWD1_GROUP_RELAYOUT != 0, TrW, Tr>::type;
+            constexpr bool WIDE = !Tr::BF16 && Tr::F * Tr::EB >= 512 && !(F512 && TG_BWD1_MAXW_F32_512 != 16);
+            using TrW = typename std::conditional<WIDE, RowTraits<T, Tr::H, Tr::D, 16>, typename tg_relayout<Tr, B256 ? TG_BWD1_MAXW_BF16_256 : F512 ? TG_BWD1_MAXW_F32_512 : 8>::type>::type;
+            using TrG = typename std::conditional<WIDE || TG_BWD1_GROUP_RELAYOUT, TrW, Tr>::type;
             static_assert(TrW::NE * TrW::LPR <= Tr::NE * Tr::LPR, "the partial workspace is sized with the default layout");
             auto launch = [&](auto tag) -> tg_status_t {
                 constexpr bool ED = decltype(tag)::value;      // delta from the edges (bf16 without the fp32 copy of O)
                 using Op = Bwd1Op<TrG, ED>;
-                using OpW0 = Bwd1Op<TrW, ED>;
+                using OpW = Bwd1Op<TrW, ED>;      // the warp tier and the hub merges may use another lane layout
                 typename Op::Params p;
                 p.Q = static_cast<const T*>(a.Q); p.K = static_cast<const T*>(a.K); p.V = static_cast<const T*>(a.V);
                 p.O = static_cast<const T*>(a.O); p.dO = static_cast<const T*>(a.dO);
@@ -136,15 +67,12 @@ struct BwdFn {
                 p.dQ = static_cast<T*>(a.dQ); p.ld = ld; p.part = dq_part;
                 p.scale = a.scale; p.scale2 = a.scale * TG_LOG2E;
                 p.O32 = a.O32;
-                if constexpr (WIDE) {
-                    return tg_launch_tiers<Op, TierPolicy<1, 2, 1, 2, 1, 16, false>, OpW0>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst");
-                } else {
-                    using OpW = typename tg_warp_op<OpW0, (TG_BWD1_MMA != 0) && ED == Tr::BF16 && MmaDotOk<TrW>::value>::type;
-                    if constexpr ((TrW::LPR == 16 && TrW::BF16) || (TrW::LPR == 32 && !TrW::BF16 && TrW::NW == 4))
-                        return tg_launch_tiers<Op, TierPolicy<TG_BWD1_U, TG_BWD1_CTAS, TG_BWD1_UP, TG_BWD1_CTASP, TG_BWD1_UW, TG_BWD1_WARPSW16, TG_BWD1_WPIPE>, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst");
-                    else
-                        return tg_launch_tiers<Op, TierPolicy<TG_BWD1_POLICY>, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst");
-                }
+                if constexpr (WIDE)
+                    return tg_launch_tiers<Op, BwdPolicyWide, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst");
+                else if constexpr ((TrW::LPR == 16 && TrW::BF16) || (TrW::LPR == 32 && !TrW::BF16 && TrW::NW == 4))
+                    return tg_launch_tiers<Op, BwdPolicyNarrow, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst");
+                else
+                    return tg_launch_tiers<Op, BwdPolicy, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_bwd/dst");
             };
             // bf16 storage: with the forward's fp32 copy of O delta = <dO, O> is taken up front (one accumulator and 16 registers
             // fewer per lane); without it delta is accumulated from the edges
@@ -152,27 +80,24 @@ struct BwdFn {
             else TG_TRY(launch(std::false_type{}));
         }
         if (which & 2) {
-            constexpr bool WIDE = !Tr::BF16 && Tr::F * Tr::EB >= 512 && !(F512 && TG_BWD2_MAXW_F32 != 16);
-            using TrW = typename std::conditional<WIDE, RowTraits<T, Tr::H, Tr::D, 16>, typename tg_relayout<Tr, B256 ? TG_BWD2_MAXW : F512 ? TG_BWD2_MAXW_F32 : 8>::type>::type;
-            using TrG = typename std::conditional<WIDE || TG_BWD2_GROUP_RELAYOUT != 0, TrW, Tr>::type;
+            constexpr bool WIDE = !Tr::BF16 && Tr::F * Tr::EB >= 512 && !(F512 && TG_BWD2_MAXW_F32_512 != 16);
+            using TrW = typename std::conditional<WIDE, RowTraits<T, Tr::H, Tr::D, 16>, typename tg_relayout<Tr, B256 ? TG_BWD2_MAXW_BF16_256 : F512 ? TG_BWD2_MAXW_F32_512 : 8>::type>::type;
+            using TrG = typename std::conditional<WIDE || TG_BWD2_GROUP_RELAYOUT, TrW, Tr>::type;
             static_assert(TrW::NE * TrW::LPR <= Tr::NE * Tr::LPR, "the partial workspace is sized with the default layout");
             using Op = Bwd2Op<TrG>;
-            using OpW0 = Bwd2Op<TrW>;
+            using OpW = Bwd2Op<TrW>;
             typename Op::Params p;
             p.Q = static_cast<const T*>(a.Q); p.K = static_cast<const T*>(a.K); p.V = static_cast<const T*>(a.V);
             p.dO = static_cast<const T*>(a.dO);
             p.t_dst = a.b->t_dst; p.ld = ld;
             p.dK = static_cast<T*>(a.dK); p.dV = static_cast<T*>(a.dV); p.part = dkv_part;
             p.scale = a.scale; p.scale2 = a.scale * TG_LOG2E;
-            if constexpr (WIDE) {
-                TG_TRY((tg_launch_tiers<Op, TierPolicy<1, 2, 1, 2, 1, 16, false>, OpW0>(p, a.b->src, a.stream, "tg_attn_fused_bwd/src")));
-            } else {
-                using OpW = typename tg_warp_op<OpW0, (TG_BWD2_MMA != 0) && MmaDotOk<TrW>::value>::type;
-                if constexpr ((TrW::LPR == 16 && TrW::BF16) || (TrW::LPR == 32 && !TrW::BF16 && TrW::NW == 4))
-                    TG_TRY((tg_launch_tiers<Op, TierPolicy<TG_BWD2_U, TG_BWD2_CTAS, TG_BWD2_UP, TG_BWD2_CTASP, TG_BWD2_UW, TG_BWD2_WARPSW16, TG_BWD2_WPIPE>, OpW>(p, a.b->src, a.stream, "tg_attn_fused_bwd/src")));
-                else
-                    TG_TRY((tg_launch_tiers<Op, TierPolicy<TG_BWD2_POLICY>, OpW>(p, a.b->src, a.stream, "tg_attn_fused_bwd/src")));
-            }
+            if constexpr (WIDE)
+                TG_TRY((tg_launch_tiers<Op, BwdPolicyWide, OpW>(p, a.b->src, a.stream, "tg_attn_fused_bwd/src")));
+            else if constexpr ((TrW::LPR == 16 && TrW::BF16) || (TrW::LPR == 32 && !TrW::BF16 && TrW::NW == 4))
+                TG_TRY((tg_launch_tiers<Op, BwdPolicyNarrow, OpW>(p, a.b->src, a.stream, "tg_attn_fused_bwd/src")));
+            else
+                TG_TRY((tg_launch_tiers<Op, BwdPolicy, OpW>(p, a.b->src, a.stream, "tg_attn_fused_bwd/src")));
         }
         return TG_OK;
     }

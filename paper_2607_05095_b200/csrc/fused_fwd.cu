@@ -1,37 +1,18 @@
 // fused_fwd.cu -- tg_attn_fused_fwd: SDDMM -> edge softmax -> alpha-weighted aggregation in one pass
 // (DESIGN.md §2, §5.3).  s and alpha never reach HBM.
 #include "dispatch.cuh"
-#include "ops_mma.cuh"
+#include "ops.cuh"
 
-// launch policy {edges per trip, min CTAs per SM} for the pipelined and the plain kernel variants
-#ifndef TG_FWD_U
-#define TG_FWD_U 2
-#endif
-#ifndef TG_FWD_CTAS
-#define TG_FWD_CTAS 2
-#endif
-#ifndef TG_FWD_UP
-#define TG_FWD_UP 2
-#endif
-#ifndef TG_FWD_CTASP
-#define TG_FWD_CTASP 3
-#endif
-#ifndef TG_FWD_UW
-#define TG_FWD_UW TG_FWD_U
-#endif
-#ifndef TG_FWD_WARPSW
-#define TG_FWD_WARPSW (8 * TG_FWD_CTAS)
-#endif
-#ifndef TG_FWD_WPIPE
-#define TG_FWD_WPIPE true
-#endif
-// 1: bf16 rows of 256 bytes with D in {16, 32}: the warp tier takes its logits from HMMA (ops_mma.cuh); 0 (default): FHFMA.
-// Measured on config 4 (profiles/r02_hmma_probe.md): parity green, 6 % fewer instructions, but 0.365 -> 0.396 ms: the
-// dependent HMMA chain (23 cycles each) and the block-diagonal padding cost more issue time than the FHFMA they replace.
-#ifndef TG_FWD_MMA
-#define TG_FWD_MMA 0
-#endif
-#define TG_FWD_POLICY TG_FWD_U, TG_FWD_CTAS, TG_FWD_UP, TG_FWD_CTASP, TG_FWD_UW, TG_FWD_WARPSW, TG_FWD_WPIPE
+// Launch policy TierPolicy<U pipelined, min CTAs/SM pipelined, U plain, min CTAs/SM plain, U warp tier, resident warps/SM of the
+// warp tier, warp tier pipelined>: two edges per trip everywhere; the values are the round-2 sweep's winners on config 4
+// (profiles/r01_other_configs_and_probes.md lists the variants: U = 1, other occupancy caps, the HMMA logits of
+// profiles/r02_hmma_probe.md -- all measured slower and no longer in the tree).
+using FwdPolicy = TierPolicy<2, 2, 2, 3, 2, 16, true>;
+using FwdPolicyNarrow = TierPolicy<2, 2, 2, 3, 2, 24, true>;   // one vector per lane (92 registers): 24 resident warps per SM
+// Words of a gathered row per lane in the warp tier: bf16 rows of 256 bytes at 4 (LPR 16, one 16-byte vector per lane: half the
+// buffer / accumulator registers of LPR 8), fp32 rows of 512 bytes at 4 (LPR 32; config 5: forward 5.98 -> 5.36 ms vs LPR 16).
+// The group tiers use the warp tier's layout too (config 3: 53.4 -> 51.3 us per step; config 4 indifferent).
+constexpr int TG_FWD_MAXW_BF16_256 = 4, TG_FWD_MAXW_F32_512 = 4;
 
 struct FwdArgs {
     const tg_block* b;
@@ -44,27 +25,11 @@ struct FwdArgs {
     float* O32;
 };
 
-#ifndef TG_FWD_GROUP_RELAYOUT
-#define TG_FWD_GROUP_RELAYOUT 1   // 1: the group tiers use the warp tier's layout too (config 3: 53.4 -> 51.3 us; config 4 indifferent)
-#endif
-#ifndef TG_FWD_MAXW
-#define TG_FWD_MAXW 4   // words of a gathered 256-byte bf16 row per lane (8: LPR 8, 4: LPR 16), see fused_bwd.cu
-#endif
-#ifndef TG_FWD_MAXW_F32
-#define TG_FWD_MAXW_F32 4   // the same knob for fp32 rows of 512 bytes: 4 = LPR 32 (config 5: forward 5.98 -> 5.36 ms), 8 = LPR 16
-#endif
-#ifndef TG_FWD_WARPSW16
-#define TG_FWD_WARPSW16 24   // resident warps per SM of the warp tier in the LPR-16 layout (92 registers)
-#endif
 template <class Tr0>
 struct FwdFn {
     static tg_status_t run(const FwdArgs& a) {
-        // group tiers: default layout (LPR 8: four rows per warp instruction); warp tier + hub merges: bf16 rows of 256 bytes in the
-        // LPR-16 layout (one vector per lane, half the buffer / accumulator registers, 24 resident warps)
-        using TrW = typename tg_relayout<Tr0, (Tr0::BF16 && Tr0::F * Tr0::EB == 256) ? TG_FWD_MAXW : (!Tr0::BF16 && Tr0::F * Tr0::EB == 512) ? TG_FWD_MAXW_F32 : 8>::type;
-        using TrG = typename std::conditional<TG_FWD_GROUP_RELAYOUT != 0, TrW, Tr0>::type;
-        using Op = FwdOp<TrG>;
-        using OpW = typename tg_warp_op<FwdOp<TrW>, (TG_FWD_MMA != 0) && MmaDotOk<TrW>::value>::type;
+        using TrW = typename tg_relayout<Tr0, (Tr0::BF16 && Tr0::F * Tr0::EB == 256) ? TG_FWD_MAXW_BF16_256 : (!Tr0::BF16 && Tr0::F * Tr0::EB == 512) ? TG_FWD_MAXW_F32_512 : 8>::type;
+        using Op = FwdOp<TrW>;
         using T = typename Tr0::T;
         typename Op::Params p;
         p.Q = static_cast<const T*>(a.Q); p.K = static_cast<const T*>(a.K); p.V = static_cast<const T*>(a.V);
@@ -75,9 +40,9 @@ struct FwdFn {
         p.scale2 = a.scale * TG_LOG2E;
         p.O32 = a.O32;
         if constexpr ((TrW::LPR == 16 && TrW::BF16) || (TrW::LPR == 32 && !TrW::BF16 && TrW::NW == 4))
-            return tg_launch_tiers<Op, TierPolicy<TG_FWD_U, TG_FWD_CTAS, TG_FWD_UP, TG_FWD_CTASP, TG_FWD_UW, TG_FWD_WARPSW16, TG_FWD_WPIPE>, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_fwd");
+            return tg_launch_tiers<Op, FwdPolicyNarrow>(p, a.b->dst, a.stream, "tg_attn_fused_fwd");
         else
-            return tg_launch_tiers<Op, TierPolicy<TG_FWD_POLICY>, OpW>(p, a.b->dst, a.stream, "tg_attn_fused_fwd");
+            return tg_launch_tiers<Op, FwdPolicy>(p, a.b->dst, a.stream, "tg_attn_fused_fwd");
     }
 };
 

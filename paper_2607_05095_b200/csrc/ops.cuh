@@ -57,12 +57,7 @@ struct FwdOp {
         bool need = false;
 #pragma unroll
         for (int u = 0; u < UNR; ++u) {
-#if defined(TG_ABLATE) && (TG_ABLATE & 2)   // diagnostic: no dot products (the K row stays a live load)
-#pragma unroll
-            for (int j = 0; j < NHL; ++j) s[u][j] = __uint_as_float((b[u].k.w[0] ^ b[u].k.w[Tr::NW - 1]) & 0x3f800000u);
-#else
             row_dot_heads(q, b[u].k, lp, s[u]);
-#endif
             const bool ok = !MASK || (pos0 + u * stride < end);
 #pragma unroll
             for (int j = 0; j < NHL; ++j) {
@@ -91,11 +86,7 @@ struct FwdOp {
                 pr[j] = tg_exp2(s[u][j] - st[j]);
                 st[NHL + j] += pr[j];
             }
-#if defined(TG_ABLATE) && (TG_ABLATE & 1)   // diagnostic: no axpy (the V row stays a live load)
-            st[2 * NHL] += pr[0] * __uint_as_float((b[u].v.w[0] ^ b[u].v.w[Tr::NW - 1]) & 0x3f800000u);
-#else
             row_axpy_heads(st + 2 * NHL, pr, b[u].v, lp);
-#endif
         }
     }
     __device__ __forceinline__ void merge(float (&a)[NS], const float (&b)[NS]) {

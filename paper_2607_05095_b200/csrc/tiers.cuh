@@ -27,15 +27,6 @@
 
 #include "rowops.cuh"
 
-// optional operator hook: end_edges(st) runs once after a work unit's edge loop, before any merge / write (an operator
-// may keep its per-head scalars in a loop-private layout, ops_mma.cuh)
-template <class Op, class = void> struct tg_has_end_edges : std::false_type {};
-template <class Op> struct tg_has_end_edges<Op, std::void_t<decltype(&Op::end_edges)>> : std::true_type {};
-template <class Op>
-__device__ __forceinline__ void tg_end_edges(Op& op, float (&st)[Op::NS1]) {
-    if constexpr (tg_has_end_edges<Op>::value) op.end_edges(st);
-}
-
 template <class Op>
 __device__ __forceinline__ void tg_warp_merge(Op& op, float (&st)[Op::NS1]) {
     using Tr = typename Op::Tr;
@@ -71,19 +62,13 @@ __device__ __forceinline__ void tg_cta_merge(Op& op, float (&st)[Op::NS1], float
     }
 }
 
-// Where an edge loop takes its row indices from: global memory (positions clamped to the row's last edge), or a chunk
-// staged in shared memory by the warp (TG_STAGE_IDX variant of the warp tier; the stage is padded with the last index, so no clamp).
+// Where an edge loop takes its row indices from: global memory, positions clamped to the row's last edge.  (A chunk staged
+// in shared memory was measured in round 2 and brought nothing on config 4: profiles/r01_other_configs_and_probes.md.)
 struct tg_idx_global {
     const int32_t* __restrict__ p;
     int last;
     __device__ __forceinline__ int operator()(int pos) const { return tg_ldg_i32(p + min(pos, last)); }
 };
-struct tg_idx_shared {
-    const int32_t* s;   // s[0] = index of position `base`
-    int base;
-    __device__ __forceinline__ int operator()(int pos) const { return s[pos - base]; }
-};
-constexpr int TG_STAGE_PAD = 64;   // the pipelined loop looks up to 5 trips (5 * U * G <= 40 positions) past the chunk's end
 
 // Plain edge loop of one group: edges pos = i0 + n*stride < end, U per trip, all loads of a trip issued
 // before its arithmetic.  Latency is hidden by the other warps (small register budget).
@@ -166,12 +151,9 @@ __device__ __forceinline__ void tg_run_edges_pipe(Op& op, float (&st)[Op::NS1], 
 #ifndef TG_WARP_CTA_WARPS
 #define TG_WARP_CTA_WARPS 1
 #endif
-#ifndef TG_STAGE_IDX
-#define TG_STAGE_IDX 0   // 1: the warp tier of a large side stages its item's index chunk in shared memory (measured, profiles/)
-#endif
 template <class Op, int U, bool PIPE>
 __device__ __forceinline__ void tg_warp_body(const typename Op::Params& p, const int4* __restrict__ items,
-                                             const int32_t* __restrict__ indptr, int n_items, int idx, int32_t* stage = nullptr) {
+                                             const int32_t* __restrict__ indptr, int n_items, int idx) {
     using Tr = typename Op::Tr;
     const int lane = threadIdx.x & 31;
     const int g = lane / Tr::LPR;
@@ -185,16 +167,8 @@ __device__ __forceinline__ void tg_warp_body(const typename Op::Params& p, const
     const int trips = (n + Tr::G * U - 1) / (Tr::G * U);
     // a trip is full for every group when its last position (group G-1, edge U-1) is inside the chunk
     const int full_until = it.y + g + ((n / (Tr::G * U)) * (Tr::G * U));
-    if (PIPE && stage != nullptr) {
-        // stage the chunk's indices (+ TG_STAGE_PAD copies of the last one for the loop's look-ahead): coalesced loads once per
-        // item instead of one index load, one clamp and one address computation per edge and trip
-        const int32_t* __restrict__ gi = op.idx_ptr();
-        for (int i = lane; i < n + TG_STAGE_PAD; i += 32) stage[i] = tg_ldg_i32(gi + min(it.y + i, it.z - 1));
-        __syncwarp();
-        tg_run_edges_pipe_from<U>(op, st, tg_idx_shared{stage, it.y}, it.y + g, it.z, Tr::G, trips, full_until);
-    } else if constexpr (PIPE) tg_run_edges_pipe<U>(op, st, it.y + g, it.z, Tr::G, trips, full_until);
+    if constexpr (PIPE) tg_run_edges_pipe<U>(op, st, it.y + g, it.z, Tr::G, trips, full_until);
     else tg_run_edges_plain<U>(op, st, it.y + g, it.z, Tr::G, trips);
-    tg_end_edges(op, st);
     tg_warp_merge(op, st);
     if (lane < Tr::LPR) {
         if (it.w < 0) op.write_final(it.x, st, true);
@@ -204,12 +178,7 @@ __device__ __forceinline__ void tg_warp_body(const typename Op::Params& p, const
 template <class Op, int U, int MIN_WARPS, bool PIPE>
 __global__ void __launch_bounds__(TG_WARP_CTA_WARPS * 32, MIN_WARPS / TG_WARP_CTA_WARPS) tg_warp_kernel(typename Op::Params p, const int4* __restrict__ items,
                                                                            const int32_t* __restrict__ indptr, int n_items) {
-#if TG_STAGE_IDX
-    __shared__ int32_t sidx[TG_WARP_CTA_WARPS][TG_CHUNK_MAX + TG_STAGE_PAD];
-    tg_warp_body<Op, U, PIPE>(p, items, indptr, n_items, blockIdx.x * TG_WARP_CTA_WARPS + (threadIdx.x >> 5), sidx[threadIdx.x >> 5]);
-#else
     tg_warp_body<Op, U, PIPE>(p, items, indptr, n_items, blockIdx.x * TG_WARP_CTA_WARPS + (threadIdx.x >> 5));
-#endif
 }
 
 // Group tier: one group per record {row, begin, end, 0}; TG_GROUP_CTA_WARPS independent warps per CTA.
@@ -233,7 +202,6 @@ __device__ __forceinline__ void tg_group_body(const typename Op::Params& p, cons
     const int trips = __reduce_max_sync(0xffffffffu, (it.z - it.y + U - 1) / U);
     if constexpr (PIPE) tg_run_edges_pipe<U>(op, st, it.y, it.z, 1, trips, it.y);
     else tg_run_edges_plain<U>(op, st, it.y, it.z, 1, trips);
-    tg_end_edges(op, st);
     if (active) op.write_final(it.x, st, true);
 }
 template <class Op, int U, int MIN_CTAS, bool PIPE>

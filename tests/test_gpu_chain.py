@@ -11,7 +11,7 @@ import numpy as np
 import pytest
 import torch
 
-from paper_2607_05095_b200 import workloads as W
+import workloads as W
 from gpu_util import H_SUM, TDT, U32, assert_close, dev, gpu_block, host
 
 pytestmark = pytest.mark.gpu

@@ -17,7 +17,7 @@ import numpy as np
 import pytest
 import torch
 
-from paper_2607_05095_b200 import workloads as W
+import workloads as W
 from gpu_util import TDT, assert_close, assert_close_budget, dev, fp32_budget, gpu_block, host, oracle_fused, run_fused, slab_source_rows
 
 pytestmark = pytest.mark.gpu

@@ -7,7 +7,7 @@ import numpy as np
 import pytest
 import torch
 
-from paper_2607_05095_b200 import workloads as W
+import workloads as W
 from gpu_util import TDT, assert_close, dev, gpu_block, host
 from test_gpu_parity import _hub_workload
 

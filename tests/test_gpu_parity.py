@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 import torch
 
-from paper_2607_05095_b200 import workloads as W
+import workloads as W
 
 from gpu_util import C_BUDGET, H_SUM, TDT, U32, assert_close, assert_close_budget, dev, fp32_budget, gpu_block, host, oracle_fused, run_fused
 
@@ -137,6 +137,25 @@ def test_block_build_long_runs_of_empty_rows(B, oracle_mod, where):
     assert gb.info()["dst_group_small"] == int((np.diff(ob.indptr) <= 8).sum())
 
 
+def test_block_build_reuses_preallocated_outputs(B, oracle_mod):
+    """block_build(reuse=...): a second build into the first one's arrays and workspace (no allocation) gives the oracle's
+    block for the NEW lists; a Block of another shape is refused."""
+    w1 = W.small_random(31, 900, 14, 300, 2, 4, shuffle=True)
+    w2 = W.small_random(31, 900, 14, 300, 2, 4, shuffle=True)
+    w2.nbr_node = (w2.nbr_node * 5 + 1) % 977                             # same shape, other neighbours
+    g = gpu_block(B, w1, 1)
+    ptrs = (g.indptr.data_ptr(), g.kv_row.data_ptr(), g.t_edge.data_ptr())
+    g2 = B.block_build(w2.R, dev(w2.root_idx), dev(w2.nbr_node), dev(w2.edge_id), dev(w2.ts), 1, reuse=g)
+    assert ptrs == (g2.indptr.data_ptr(), g2.kv_row.data_ptr(), g2.t_edge.data_ptr()) and not g.handle
+    ob = _oblock(oracle_mod, w2, 1)
+    assert g2.U == ob.U
+    for name in ("indptr", "perm", "kv_row", "uniq_node", "t_indptr", "t_edge", "t_dst", "eid_csr", "ts_csr"):
+        assert np.array_equal(host(getattr(g2, name)), getattr(ob, name)), name
+    w3 = W.small_random(32, 901, 14, 300, 2, 4, shuffle=True)
+    with pytest.raises(ValueError):
+        B.block_build(w3.R, dev(w3.root_idx), dev(w3.nbr_node), dev(w3.edge_id), dev(w3.ts), 1, reuse=g2)
+
+
 def test_block_build_negative_ids_and_empty(B, oracle_mod):
     w = W.small_random(7, 50, 9, 30, 2, 4, shuffle=True)
     w.nbr_node = w.nbr_node - 100                           # negative node ids: full 64-bit key sort
@@ -198,7 +217,9 @@ def test_fused_all_tiers_with_hubs(B, oracle_mod, H, D, dtype):
 
 @pytest.mark.parametrize("scale", [1.0, 1e4])
 def test_fused_degree_thresholds_and_large_logits(B, oracle_mod, scale):
-    """degrees straddling every internal threshold (8/9, 256/257, 8192/8193) and logits x 1e4 (max subtraction)."""
+    """A spread of degrees from 0 to 16385 (group tier, warp tier, hub rows of up to 257 chunks on this launch-bound side) and
+    logits x 1e4 (max subtraction).  The schedule's own thresholds are straddled one by one in
+    test_fused_straddles_every_schedule_threshold below."""
     degs = [0, 1, 2, 7, 8, 9, 10, 255, 256, 257, 258, 8191, 8192, 8193, 16384, 16385]
     H, D = 2, 64
     root = np.repeat(np.arange(len(degs), dtype=np.int32), degs)
@@ -221,6 +242,55 @@ def test_fused_degree_thresholds_and_large_logits(B, oracle_mod, scale):
             assert_close_budget(f"thresholds[scale={scale:g}].{n}", g, r_, "f32", bud[n])
         else:
             assert_close(n, g, r_, "f32")
+
+
+def _straddle(*thresholds):
+    return sorted({d for t in thresholds for d in (t - 1, t, t + 1) if d >= 0})
+
+
+@pytest.mark.parametrize("side", ["launch_bound", "large"])
+def test_fused_straddles_every_schedule_threshold(B, oracle_mod, side):
+    """Destination AND source degrees at t-1, t, t+1 for every threshold of the schedule the block actually got
+    (tg_block_sched_info): the degree classes (2, 4, 8, 16, 32, 64), the side's group-tier limit, one warp item
+    (chunk), the direct hub merge (TG_HUB_DIRECT = 32 chunks) and beyond.  'launch_bound': a side below 2^20 edges
+    (group limit 32, chunk 64, one CTA per hub); 'large': >= 2^20 edges (group limit 64, forked tiers, two-level hub merge)."""
+    rng = np.random.default_rng(17)
+    if side == "launch_bound":
+        H, D, dtype, group_max, chunk, filler = 2, 64, "f32", 32, 64, (0, 0)
+    else:
+        H, D, dtype, group_max, chunk, filler = 8, 16, "bf16", 64, 128, (4000, 260)
+    degs = _straddle(1, 2, 4, 8, 16, 32, 64, group_max, chunk, 2 * chunk, 32 * chunk, 33 * chunk) + [0, 0, 3 * 32 * chunk + 5]
+    dst_deg = np.array(degs + [filler[1]] * filler[0])
+    E = int(dst_deg.sum())
+    src_deg = np.array([d for d in degs if d > 0])
+    assert src_deg.sum() <= E
+    rest = E - int(src_deg.sum())                                     # the remaining edges go to sources of degree ~ 3 and ~ 40
+    extra = []
+    while rest > 0:
+        d = min(rest, int(rng.choice([1, 2, 3, 5, 40])))
+        extra.append(d); rest -= d
+    src_deg = np.concatenate([src_deg, np.array(extra, dtype=np.int64)])
+    root = np.repeat(np.arange(len(dst_deg), dtype=np.int32), dst_deg)
+    nbr = rng.permutation(np.repeat(np.arange(len(src_deg), dtype=np.int64) * 3 + 11, src_deg))
+    w = W.Workload("straddle_" + side, 97, 17, len(dst_deg), H, D, dtype, 1.0, 1, root, nbr, np.arange(E, dtype=np.int64),
+                   rng.random(E, dtype=np.float32))
+    ob = _oblock(oracle_mod, w)
+    gb = gpu_block(B, w)
+    sched = gb.sched_info()
+    assert (E >= (1 << 20)) == (side == "large")
+    for k in ("dst", "src"):                                           # the thresholds this test was written against
+        assert sched[k + "_group_max"] == group_max and sched[k + "_chunk"] == chunk, sched
+        assert sched[k + "_hubs"] >= 9 and sched[k + "_max_deg"] == 3 * 32 * chunk + 5
+    assert np.array_equal(np.sort(np.diff(ob.t_indptr)), np.sort(src_deg))
+    feats = w.features(ob.U)
+    got = run_fused(B, gb, w, feats, 1.0)
+    ref = oracle_fused(oracle_mod, ob, feats, 1.0)
+    bud = fp32_budget(oracle_mod, ob.indptr, ob.kv_row, ob.U, feats, 1.0) if dtype == "f32" else {}
+    for n, g, r_ in zip(("O", "LSE", "dQ", "dK", "dV"), got, ref):
+        if n in bud:
+            assert_close_budget(f"straddle[{side}].{n}", g, r_, dtype, bud[n])
+        else:
+            assert_close(f"straddle[{side}].{n}", g, r_, dtype)
 
 
 def test_fused_identity_rows_and_single_source(B, oracle_mod):

@@ -12,7 +12,7 @@ import pytest
 import torch
 
 from oracle import sampler_oracle as S
-from paper_2607_05095_b200 import workloads as W
+import workloads as W
 from gpu_util import dev, host
 
 pytestmark = pytest.mark.gpu

@@ -20,14 +20,20 @@ def L():
     return binding.lib()
 
 
+def _headers_text():
+    """include/fasttg.h (the boundary) and include/fasttg_diag.h (exported diagnostics)."""
+    inc = os.path.join(ROOT, "include")
+    return "\n".join(open(os.path.join(inc, n)).read() for n in sorted(os.listdir(inc)) if n.endswith(".h"))
+
+
 def _declared():
-    text = open(os.path.join(ROOT, "include", "fasttg.h")).read()
+    text = _headers_text()
     return sorted(set(re.findall(r"TG_API\s+[\w\s\*]+?\b(tg_\w+)\s*\(", text)))
 
 
 def _signatures_from_header():
     """name -> (result, arguments) in binding.SIGNATURES' letters, read off the declarations of include/fasttg.h."""
-    text = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "fasttg.h")).read(), flags=re.S)
+    text = re.sub(r"/\*.*?\*/", "", _headers_text(), flags=re.S)
     scalar = {"int": "I", "tg_dtype_t": "I", "tg_status_t": "I", "int64_t": "L", "uint64_t": "Q", "unsigned long long": "Q",
               "size_t": "Z", "float": "F", "double": "D", "tg_stream_t": "P"}
 
@@ -61,8 +67,8 @@ def test_every_declared_symbol_is_exported(L):
     names = _declared()
     assert len(names) >= 20 and "tg_attn_fused_fwd" in names and "tg_block_build" in names and "tg_launch_count" in names
     for n in names:
-        assert hasattr(L, n), f"{n} declared in include/fasttg.h but not exported by libfasttg.so"
-    assert sorted(binding.EXPORTS) == names, "binding.EXPORTS and include/fasttg.h disagree"
+        assert hasattr(L, n), f"{n} declared in include/*.h but not exported by libfasttg.so"
+    assert sorted(binding.EXPORTS) == names, "binding.EXPORTS and include/*.h disagree"
 
 
 def test_host_only_entry_points(L):
@@ -127,3 +133,34 @@ def test_reference_arm_runs_on_rank0_only():
     line = json.loads(r0.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["cpu_baseline"]["kind"] == "oracle" and line["value"] > 0
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["unit"] == "edges/s"
+
+
+def test_bench_gpus_n_starts_n_ranks_itself():
+    """`python bench.py --gpus 2` without a rendezvous in the environment launches two ranks (torch.distributed.run on
+    127.0.0.1).  Reference arm: rank 0 alone prints the line, with n_gpus = 2.  Own arm on a box without a GPU: both ranks start
+    and the job fails with the no-CPU-fallback message (on a GPU box this leg is covered by the driver's scaling run)."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    base = [sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1", "--warmup", "0", "--config", "1"]
+    r = subprocess.run(base + ["--impl", "reference"], env=env, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, r.stdout
+    line = json.loads(lines[0])
+    assert line["impl"] == "reference" and line["n_gpus"] == 2 and line["value"] > 0
+    import torch
+    if not torch.cuda.is_available():
+        r = subprocess.run(base, env=env, capture_output=True, text=True, timeout=600)
+        both = r.stdout + r.stderr
+        assert r.returncode != 0
+        # both ranks were started; at least one got as far as the refusal (the launcher stops the other rank as soon as the
+        # first one fails, so the second message is a race and is not asserted)
+        assert "rank 0/2 started" in both and "rank 1/2 started" in both, both[-3000:]
+        assert "bench.py needs a CUDA device" in both, both[-3000:]
+
+
+def test_step_spread_statistics():
+    sys.path.insert(0, ROOT)
+    import bench
+    sp = bench.step_spread([3.0, 1.0, 2.0, 10.0, 2.0], "unit test")
+    assert sp["median"] == 2.0 and sp["min"] == 1.0 and sp["max"] == 10.0 and sp["n"] == 5 and sp["p10"] <= sp["median"] <= sp["p90"]
+    assert bench.step_spread([], "empty") is None

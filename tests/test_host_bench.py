@@ -9,7 +9,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 sys.path.insert(0, ROOT)
 import bench  # noqa: E402
-from paper_2607_05095_b200 import workloads as W  # noqa: E402
+import workloads as W  # noqa: E402
 
 
 def test_call_bytes_partition_the_compulsory_bytes():

@@ -12,7 +12,7 @@ import numpy as np
 import pytest
 import torch
 
-from paper_2607_05095_b200 import workloads as W
+import workloads as W
 
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
 RTOL, ATOL = 1e-10, 1e-12

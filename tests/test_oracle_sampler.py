@@ -16,7 +16,7 @@ import numpy as np
 import pytest
 
 from oracle import sampler_oracle as S
-from paper_2607_05095_b200 import workloads as W
+import workloads as W
 
 
 def _tiny_stream(seed, n_nodes=7, m=60):
