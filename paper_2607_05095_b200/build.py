@@ -39,7 +39,7 @@ def _nvcc() -> str:
 
 def _stamp() -> str:
     h = hashlib.sha256()
-    h.update(" ".join(NVCC_FLAGS).encode())
+    h.update(" ".join(NVCC_FLAGS).replace(ROOT, "<root>").encode())   # independent of where the checkout lives
     names = sorted(os.listdir(CSRC))
     for n in names:
         p = os.path.join(CSRC, n)
